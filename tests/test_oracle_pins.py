@@ -1,0 +1,342 @@
+"""Pins P1..P11 of SURVEY.md 8(c): the fp64 oracle against what mathematics fixes.
+
+None of these touch the CUDA path.  Expected values come from tests/golden (transcribed from
+SURVEY.md Appendix A/B, computed there by independent scripts), from closed forms, from counting
+arguments, or from the O(N^2) plain definition on tiny inputs.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from conftest import fnum, golden_lines
+from paper_1411_3396_b200 import workloads
+
+BOX16 = (16.0, 16.0, 16.0)
+
+
+def _two(oracle, d, eps, box=(32.0, 32.0, 32.0), at=(5.0, 7.0, 9.0), axis=0, m2=1.0):
+    p = np.zeros((2, 4), dtype=np.float32)
+    p[:, :3] = at
+    p[1, axis] += d
+    p[:, 3] = (1.0, m2)
+    return p, oracle.make_params(box, 3.0, eps)
+
+
+# ---------------------------------------------------------------- P1, P2, P9, P10 ----
+
+def test_p1_two_particle_closed_form(oracle_mod):
+    """30 printed values of f and a = d*f (softening, polynomial, force law)."""
+    rows = golden_lines("p1_two_particle.txt")
+    assert len(rows) == 30
+    for d, eps, f_exp, a_exp in rows:
+        d, eps, f_exp, a_exp = float(d), float(eps), float(f_exp), float(a_exp)
+        prm = oracle_mod.make_params((32.0,) * 3, 3.0, eps)
+        # the fp32 eps is what the oracle sees; golden values used the decimal eps: allow that gap
+        tol = 2e-7 * abs(f_exp) + 1e-15
+        assert abs(oracle_mod.pair_factor(prm, d * d) - f_exp) <= tol
+        # through the full pair-sum code, both brute force and cell list, exactly representable d only
+        if d in (0.5, 1.0, 1.5, 2.0, 2.5):
+            pos, prm = _two(oracle_mod, d, eps)
+            for acc in (oracle_mod.accel_bruteforce(pos, prm), oracle_mod.accel(pos, prm)):
+                assert abs(acc[0, 0] - a_exp) <= 2e-7 * abs(a_exp)
+                assert abs(acc[1, 0] + a_exp) <= 2e-7 * abs(a_exp)   # Newton's third law, m = 1
+                assert acc[0, 1] == 0.0 and acc[0, 2] == 0.0
+
+
+def test_p1_sign_and_mass(oracle_mod):
+    """The first particle is pulled TOWARDS the second; acceleration scales with the OTHER mass (R2, R14)."""
+    for axis in range(3):
+        pos, prm = _two(oracle_mod, 1.0, 0.1, axis=axis, m2=3.0)
+        acc = oracle_mod.accel(pos, prm)
+        assert acc[0, axis] > 0 and acc[1, axis] < 0
+        assert abs(acc[0, axis] / acc[1, axis] + 3.0) < 1e-12
+        other = [a for a in range(3) if a != axis]
+        assert np.all(acc[:, other] == 0.0)
+
+
+def test_p2_zero_beyond_cutoff(oracle_mod):
+    """Pairs at exactly rc and beyond contribute nothing (strict <, R5); just inside they do."""
+    for d in (3.0, 3.0000002, 3.5, 4.75, 10.0):
+        pos, prm = _two(oracle_mod, d, 0.1)
+        for acc in (oracle_mod.accel_bruteforce(pos, prm), oracle_mod.accel(pos, prm)):
+            assert np.all(acc == 0.0), d
+    pos, prm = _two(oracle_mod, 2.9999998, 0.1, at=(1.0, 7.0, 9.0))   # 1 + 2.9999998 -> 3.99999976 in fp32
+    assert float(pos[1, 0]) - float(pos[0, 0]) < 3.0
+    assert oracle_mod.accel(pos, prm)[0, 0] != 0.0
+    assert oracle_mod.pair_factor(prm, 9.0) == 0.0
+    assert oracle_mod.pair_factor(prm, math.nextafter(9.0, 0.0)) != 0.0
+
+
+def test_p9_p10_default_polynomial(oracle_mod):
+    """Coefficient table: bit patterns, re-derivation, P(0) = c0, P(9) = 1/27 - 5.7e-9, cutoff jumps (R6)."""
+    from oracle import default_poly
+    rows = golden_lines("poly_default.txt")
+    bits = [int(r[2], 16) for r in rows]
+    assert tuple(bits) == tuple(oracle_mod.DEFAULT_POLY_BITS)
+    c64, c32, q = default_poly.derive()
+    assert [int(v) for v in c32.view(np.uint32)] == bits                      # P10
+    for k, r in enumerate(rows):
+        assert abs(c64[k] - float(r[1])) <= 2e-12 * abs(float(r[1]))
+    prm = oracle_mod.make_params((32.0,) * 3, 3.0, 0.1)
+    assert oracle_mod.poly(prm, 0.0) == float(oracle_mod.DEFAULT_POLY[0])     # P(0) = c0
+    assert abs((oracle_mod.poly(prm, 9.0) - 1.0 / 27.0) + 5.7e-9) < 1e-10      # P9
+    # R6: jump at the cutoff is only the softening term
+    for eps, jump in ((0.1, -6.16e-5), (0.05, -1.54e-5), (0.02, -2.46e-6)):
+        prm = oracle_mod.make_params((32.0,) * 3, 3.0, eps)
+        f = oracle_mod.pair_factor(prm, math.nextafter(9.0, 0.0))
+        assert abs(f - jump) < 0.01 * abs(jump)
+    # fit quality quoted in Appendix A
+    s = np.linspace(0, 9, 4001)
+    P = np.polynomial.polynomial.polyval(s, c32.astype(np.float64))
+    assert abs(np.max(np.abs(P - default_poly.gauss_filtered_force(s))) - 4.15e-4) < 2e-6
+
+
+def test_polynomial_is_runtime_input(oracle_mod):
+    """poly[6] is data (R4): with P = 0 the pair factor is pure Plummer; with P = const it shifts."""
+    prm = oracle_mod.make_params((32.0,) * 3, 3.0, 0.25, poly=np.zeros(6))
+    for s in (0.0, 0.3, 4.0, 8.9):
+        assert abs(oracle_mod.pair_factor(prm, s) - (s + 0.0625) ** -1.5) < 1e-14 * (s + 0.0625) ** -1.5
+    prm = oracle_mod.make_params((32.0,) * 3, 3.0, 0.25, poly=[0.5, 0, 0, 0, 0, 0.25])
+    assert abs(oracle_mod.pair_factor(prm, 2.0) - ((2.0625) ** -1.5 - 0.5 - 0.25 * 32.0)) < 1e-13
+
+
+# ---------------------------------------------------------------- P3, P4, P11 ----
+
+def test_p3_unit_lattice(oracle_mod):
+    """Perfect lattice: exactly 92 in-cutoff neighbours per site with the strict cutoff, zero net force.
+
+    SURVEY.md Appendix B (P3) prints "122 with <, 152 with <=".  Counting integer vectors shows the
+    shells are 92 (0 < |v|^2 < 9) and 122 (<= 9): the 30 vectors of squared length 9 are the difference.
+    The survey's own sum |f d| = 8.00847 is the 92-neighbour sum, so its count is a slip of one shell;
+    mathematics decides (reading R5)."""
+    pos = workloads.unit_lattice(12)
+    prm = oracle_mod.make_params((12.0,) * 3, 3.0, 0.1)
+    acc, st = oracle_mod.accel(pos, prm, stats=True)
+    assert np.all(st["n_in"] == 92)
+    assert np.max(np.abs(acc)) < 2e-14
+    assert abs(st["sum_abs"][0] - 8.00847) < 1e-5       # Appendix B, P3: scale of the cancelling terms
+    # brute force agrees on the count (122 would appear with <=: 30 vectors of squared length 9)
+    accb, n_in, _ = oracle_mod.accel_bruteforce(pos[:, :], prm, stats=True)
+    assert np.all(n_in == 92) and np.max(np.abs(accb)) < 2e-14
+    v = np.array([(i, j, k) for i in range(-3, 4) for j in range(-3, 4) for k in range(-3, 4)])
+    s = (v * v).sum(1)
+    assert (s == 9).sum() == 30 and ((s > 0) & (s < 9)).sum() == 92 and ((s > 0) & (s <= 9)).sum() == 122
+
+
+def test_p4_momentum_conservation(oracle_mod):
+    """sum_i m_i a_i = 0 (pair antisymmetry; no neighbour cell missed or double counted)."""
+    rng = np.random.default_rng(7)
+    for box in ((16.0, 16.0, 16.0), (9.6, 12.8, 19.2)):
+        n = 3000
+        pos = np.empty((n, 4), dtype=np.float32)
+        pos[:, :3] = rng.random((n, 3)) * np.asarray(box)
+        pos[:, 3] = rng.uniform(0.5, 2.0, n)
+        prm = oracle_mod.make_params(box, 3.0, 0.05)
+        acc, st = oracle_mod.accel(pos, prm, stats=True)
+        m = pos[:, 3].astype(np.float64)
+        net = (m[:, None] * acc).sum(0)
+        scale = (m * st["sum_abs"]).sum()
+        assert np.max(np.abs(net)) <= 1e-13 * scale
+
+
+def test_p11_permutation_invariance(oracle_mod):
+    rng = np.random.default_rng(11)
+    pos, box = workloads.scaled_clustered(2500, (4, 4, 4), seed=5, frac_halo=0.5, n_halo=3)
+    prm = oracle_mod.make_params(box, 3.0, 0.05)
+    a0 = oracle_mod.accel(pos, prm)
+    p = rng.permutation(pos.shape[0])
+    a1 = oracle_mod.accel(pos[p], prm)
+    scale = np.linalg.norm(a0, axis=1).max()
+    assert np.max(np.abs(a1 - a0[p])) <= 1e-12 * scale
+
+
+# ---------------------------------------------------------------- P5, P6 ----
+
+def test_p5_eight_particle_example(oracle_mod):
+    rows = golden_lines("p5_eight_particles.txt")
+    pos = np.array([[float(t) for t in r[:4]] for r in rows], dtype=np.float32)
+    n_exp = np.array([int(r[4]) for r in rows])
+    a_exp = np.array([[float(t) for t in r[5:8]] for r in rows])
+    prm = oracle_mod.make_params(BOX16, 3.0, 0.1)
+    for acc, n_in in ((oracle_mod.accel(pos, prm, stats=True)[0], oracle_mod.accel(pos, prm, stats=True)[1]["n_in"]),
+                      oracle_mod.accel_bruteforce(pos, prm, stats=True)[:2]):
+        assert np.array_equal(n_in, n_exp)
+        assert np.all(np.abs(acc - a_exp) <= 3e-7 * np.abs(a_exp) + 1e-18)
+    net = (pos[:, 3:4].astype(np.float64) * oracle_mod.accel(pos, prm)).sum(0)
+    assert np.max(np.abs(net)) < 1e-14
+
+
+@pytest.mark.parametrize("ncell,kind,seed", [((3, 3, 3), "uniform", 1), ((4, 3, 5), "uniform", 2),
+                                             ((5, 5, 5), "clustered", 3), ((3, 4, 3), "clustered", 4),
+                                             ((2, 2, 2), "uniform", 5)])
+def test_p6_bruteforce_vs_cell_list(oracle_mod, ncell, kind, seed):
+    """The oracle's own neighbour search against the O(N^2) plain definition, N <= 4096."""
+    n = 1500 if kind == "uniform" else 4096
+    pos, box = workloads.scaled_clustered(n, ncell, seed=seed, frac_halo=0.0 if kind == "uniform" else 0.6,
+                                          n_halo=0 if kind == "uniform" else 4, a_range=(0.2, 1.5))
+    rng = np.random.default_rng(seed)
+    pos[:, 3] = rng.uniform(0.5, 1.5, pos.shape[0]).astype(np.float32)
+    prm = oracle_mod.make_params(box, 3.0, 0.05)
+    a_bf, n_bf, s_bf = oracle_mod.accel_bruteforce(pos, prm, stats=True)
+    a_cl, st = oracle_mod.accel(pos, prm, stats=True)
+    assert np.array_equal(n_bf, st["n_in"])
+    assert np.max(np.abs(a_bf - a_cl)) <= 1e-12 * np.max(s_bf)
+    # subset evaluation returns the same rows
+    sub = rng.choice(pos.shape[0], 97, replace=False)
+    assert np.array_equal(oracle_mod.accel(pos, prm, targets=sub), a_cl[sub])
+
+
+def test_independent_python_pair_sum(oracle_mod):
+    """A second, independent statement of the definition (pure numpy, fp64, all-pairs with np.round
+    minimum image) on 300 particles."""
+    rng = np.random.default_rng(3)
+    box = np.array([9.6, 9.6, 12.8])
+    n = 300
+    pos = np.empty((n, 4), dtype=np.float32)
+    pos[:, :3] = rng.random((n, 3)) * box
+    pos[:, 3] = rng.uniform(0.5, 2.0, n)
+    eps = 0.07
+    prm = oracle_mod.make_params(box, 3.0, eps)
+    x = pos[:, :3].astype(np.float64)
+    Lf = np.array([np.float32(b) for b in box], dtype=np.float64)
+    d = x[None, :, :] - x[:, None, :]
+    d -= Lf * np.round(d / Lf)
+    s = (d * d).sum(-1)
+    c = oracle_mod.DEFAULT_POLY.astype(np.float64)
+    P = sum(c[k] * s ** k for k in range(6))
+    e2 = float(np.float32(eps)) ** 2
+    f = (s + e2) ** -1.5 - P
+    f[(s >= 9.0) | np.eye(n, dtype=bool)] = 0.0
+    a = ((pos[:, 3].astype(np.float64)[None, :] * f)[:, :, None] * d).sum(1)
+    got = oracle_mod.accel(pos, prm)
+    assert np.max(np.abs(got - a)) <= 1e-11 * np.abs(a).max()
+
+
+# ---------------------------------------------------------------- P7 ----
+
+def _config1_matches_golden():
+    rows = golden_lines("p7_config1.txt")
+    pos = workloads.generate(1)
+    for r in rows:
+        if r[0] == "x":
+            i = int(r[1])
+            if not all(float(pos[i, a]) == fnum(r[2 + a]) for a in range(3)):
+                return None, rows
+    return pos, rows
+
+
+def test_p7_config1_soft_pins(oracle_mod):
+    pos, rows = _config1_matches_golden()
+    if pos is None:
+        pytest.skip("this numpy does not reproduce SURVEY.md's config-1 stream (soft pin)")
+    w = workloads.CONFIGS[1]
+    prm = oracle_mod.make_params(w.box, w.rcut, w.eps)
+    acc, st = oracle_mod.accel(pos, prm, stats=True)
+    kv = {r[0]: r[1:] for r in rows if r[0] != "x"}
+    assert int(st["n_in"].sum()) == int(kv["pairs"][0])
+    na = np.linalg.norm(acc, axis=1)
+    assert abs(math.sqrt(np.mean(na * na)) - float(kv["rms"][0])) < 1e-6
+    # golden values were computed with the decimal eps = 0.1; the C ABI carries eps as fp32
+    # (0.1f = 0.1 * (1 + 1.5e-8)), which moves close-pair forces by a few 1e-8 relative
+    assert abs(np.sum(na * na) / float(kv["sumsq"][0]) - 1.0) < 1e-7
+    for r in rows:
+        if r[0] == "x":
+            i = int(r[1])
+            exp = np.array([float(t) for t in r[5:8]])
+            assert np.all(np.abs(acc[i] - exp) <= 1e-7 * np.abs(exp).max())
+    cs, perm, srt = oracle_mod.build_mesh(pos, w.box, w.ncell)
+    assert [int(v) for v in np.diff(cs)[:5]] == [int(v) for v in kv["occ"]]
+    assert [int(v) for v in perm[:8]] == [int(v) for v in kv["perm"]]
+    # candidate pairs W of the chaining mesh: sum_c n_c * sum_{27 stencil} n_c'
+    cnt = np.diff(cs).astype(np.int64).reshape(w.ncell[2], w.ncell[1], w.ncell[0])
+    sten = sum(np.roll(cnt, (dz, dy, dx), axis=(0, 1, 2)) for dz in (-1, 0, 1) for dy in (-1, 0, 1)
+               for dx in (-1, 0, 1))
+    assert int((cnt * sten).sum()) == int(kv["W"][0])
+
+
+# ---------------------------------------------------------------- P8 binning ----
+
+def test_p8_binning_worked_example(oracle_mod):
+    rows = golden_lines("p8_binning.txt")
+    pts = [r for r in rows if r[0].isdigit()]
+    pos = np.zeros((len(pts), 4), dtype=np.float32)
+    for r in pts:
+        pos[int(r[0]), :3] = [np.float32(fnum(t)) for t in r[1:4]]
+    pos[:, 3] = 1.0
+    cid_exp = np.array([int(r[7]) for r in pts], dtype=np.uint32)
+    cxyz = np.array([[int(t) for t in r[4:7]] for r in pts])
+    assert np.array_equal(cid_exp, cxyz[:, 0] + 5 * (cxyz[:, 1] + 5 * cxyz[:, 2]))
+    ncell = (5, 5, 5)
+    assert np.array_equal(oracle_mod.cell_ids(pos, BOX16, ncell), cid_exp)
+    cs, perm, srt = oracle_mod.build_mesh(pos, BOX16, ncell)
+    perm_exp = np.array([int(t) for t in next(r for r in rows if r[0] == "perm")[1:]], dtype=np.uint32)
+    assert np.array_equal(perm, perm_exp)
+    assert np.array_equal(cid_exp[perm], [int(t) for t in next(r for r in rows if r[0] == "sorted_cid")[1:]])
+    cs_exp = np.zeros(126, dtype=np.uint32)
+    for r in rows:
+        if r[0] == "cs":
+            cs_exp[int(r[1]): int(r[2]) + 1] = int(r[3])
+    assert np.array_equal(cs, cs_exp)
+    assert np.array_equal(srt, pos[perm])
+    for r in rows:
+        if r[0] == "r10":
+            x, box, nc, cell = fnum(r[1]), float(r[2]), int(r[3]), int(r[4])
+            p = np.array([[x, 0, 0, 1]], dtype=np.float32)
+            assert int(oracle_mod.cell_ids(p, (box,) * 3, (nc,) * 3)[0]) == cell
+            assert math.floor(float(np.float32(x)) * nc / box) == cell - 1   # exact arithmetic differs
+
+
+def test_binning_invariants_and_domain(oracle_mod):
+    pos, box = workloads.scaled_clustered(20000, (6, 5, 7), seed=9, frac_halo=0.7, n_halo=5)
+    ncell = (6, 5, 7)
+    cid = oracle_mod.cell_ids(pos, box, ncell)
+    cs, perm, srt = oracle_mod.build_mesh(pos, box, ncell)
+    n = pos.shape[0]
+    assert np.array_equal(np.sort(perm), np.arange(n, dtype=np.uint32))          # a permutation
+    key = cid[perm]
+    assert np.all(np.diff(key.astype(np.int64)) >= 0)                           # keys non-decreasing
+    same = key[1:] == key[:-1]
+    assert np.all(perm[1:][same] > perm[:-1][same])                             # stable inside a cell
+    assert np.array_equal(cs, np.concatenate([[0], np.cumsum(np.bincount(cid, minlength=210))]))
+    assert np.array_equal(perm, np.argsort(cid, kind="stable").astype(np.uint32))  # library routine
+    assert np.array_equal(srt, pos[perm])
+    for bad in (-1e-3, 19.2, np.nan, np.inf):
+        q = pos[:4].copy()
+        q[2, 0] = bad
+        with pytest.raises(ValueError):
+            oracle_mod.cell_ids(q, box, ncell)
+
+
+# ---------------------------------------------------------------- kick / stream ----
+
+def test_kick_and_stream(oracle_mod):
+    rng = np.random.default_rng(5)
+    n = 1000
+    v = rng.normal(size=(n, 4)).astype(np.float32)
+    a = rng.normal(size=(n, 4)).astype(np.float32) * 50
+    kdt = np.float32(0.01)
+    v1 = oracle_mod.kick(v, a, kdt)
+    exact = v[:, :3].astype(np.float64) + a[:, :3].astype(np.float64) * float(kdt)   # exact in fp64? no: rounds once
+    assert np.array_equal(v1[:, 3], v[:, 3])
+    assert np.all(np.abs(v1[:, :3] - exact) <= np.spacing(np.abs(v1[:, :3])) * 0.5 + 1e-30)
+    # 5 fused steps on fixed a (R16 config-4 reading)
+    v5 = v.copy()
+    for _ in range(5):
+        v5 = oracle_mod.kick(v5, a, kdt)
+    assert np.max(np.abs(v5[:, :3] - (v[:, :3] + 5 * float(kdt) * a[:, :3].astype(np.float64)))) < 1e-4
+    box = (16.0, 16.0, 32.0)
+    x = np.empty((n, 4), dtype=np.float32)
+    x[:, :3] = rng.random((n, 3)) * np.asarray(box)
+    x[:, 3] = 1.0
+    x[0, 0], v[0, 0] = 15.999999, 1.0          # crosses +L
+    x[1, 0], v[1, 0] = 0.0, -1.0               # crosses 0
+    x[2, 2], v[2, 2] = 0.0, -1e-9              # -tiny + L rounds to L -> must become 0
+    x1 = oracle_mod.stream(x, v, 0.5, box)
+    assert np.all(x1[:, :3] >= 0) and np.all(x1[:, :3] < np.asarray(box, dtype=np.float32))
+    assert x1[2, 2] == 0.0
+    assert abs(x1[0, 0] - 0.499999) < 1e-5 and abs(x1[1, 0] - 15.5) < 1e-6
+    d = (x1[:, :3].astype(np.float64) - x[:, :3] - 0.5 * v[:, :3].astype(np.float64))
+    d -= np.asarray(box) * np.round(d / np.asarray(box))
+    assert np.max(np.abs(d)) < 4e-6
+    oracle_mod.cell_ids(x1, box, (5, 5, 10))   # stays in the domain
