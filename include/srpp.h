@@ -1,0 +1,133 @@
+/*
+ * srpp.h -- C ABI of the B200-native short-range particle-particle (PP) force solver.
+ *
+ * The hot path of HACC's short-range solver as the paper names it for accelerated systems
+ * (PAPER.md = arXiv:1411.3396, Heitmann et al., "The Q Continuum Simulation"):
+ *   PAPER.md:63 (Sec. 2)    force = long-range spectrally filtered PM + short-range solver; on
+ *                           accelerated systems the short-range solver is a direct particle-particle
+ *                           ("N^2") sum, i.e. "compute intensive".
+ *   PAPER.md:65 (Sec. 2)    spectral filtering pushes the PM / short-range "hand-over" to small scales:
+ *                           the pair force is Newtonian minus the filtered grid force, zero beyond rc.
+ *   PAPER.md:73 (Sec. 2.1)  a "short-range force timestep" updates the particles (the kick).
+ * PAPER.md prints no formula for this path; BASELINE.json `north_star` fixes its form and SURVEY.md 8(c)
+ * lists the readings R1..R18 (repeated in DESIGN.md) that make it precise:
+ *
+ *   a_i = sum_{j, s_ij < rc^2}  m_j d_ij [ (s_ij + eps^2)^(-3/2) - P(s_ij) ],     s_ij = |d_ij|^2,
+ *   d_ij = minimum image of x_j - x_i in the periodic box,  P(s) = sum_{k=0..5} poly[k] s^k,  G = 1.
+ *
+ * Conventions
+ *   - Every array argument is a DEVICE pointer unless its name ends in `_host`.  float4 arrays are
+ *     AoS (x, y, z, w), 16-byte aligned.  The caller owns all arrays and the workspace; the library
+ *     owns only the small host-side context.  No call allocates device memory.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (0 = the legacy default stream).  Calls enqueue
+ *     work on it and return; only srpp_build_mesh() synchronises the stream (it reads a device-side
+ *     error flag), and the *_host convenience entry points synchronise because they copy.
+ *   - Every call returns SRPP_OK (0) or a negative srpp_status; nothing throws or aborts across the ABI.
+ *     There is no CPU fallback and no other back end: without a CUDA device every compute call
+ *     returns SRPP_ERR_CUDA.
+ *   - Units: PM grid units, G = 1, accelerations (no m_i factor).
+ */
+#ifndef SRPP_H_
+#define SRPP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SRPP_VERSION 1
+
+typedef enum {
+  SRPP_OK = 0,
+  SRPP_ERR_INVALID_ARG = -1, /* null pointer, n < 0 or n >= 2^31, eps <= 0, rcut <= 0, non-finite parameter   */
+  SRPP_ERR_GEOMETRY = -2,    /* ncell < 3 on an axis, box/ncell < rcut, or more than 2^24 cells (R8)          */
+  SRPP_ERR_DOMAIN = -3,      /* a position outside [0, L) or not finite, found while binning (R13)            */
+  SRPP_ERR_WORKSPACE = -4,   /* workspace too small or not 256-byte aligned                                   */
+  SRPP_ERR_STATE = -5,       /* srpp_accel before a successful srpp_build_mesh, or n mismatch                 */
+  SRPP_ERR_CUDA = -6         /* CUDA runtime error (text of the last one: srpp_last_cuda_error)                */
+} srpp_status;
+
+/* Solver parameters (plain data; copied by srpp_create). */
+typedef struct {
+  float box[3];      /* periodic box lengths Lx, Ly, Lz (> 0), grid units                                   */
+  int32_t ncell[3];  /* chaining-mesh cells per axis (>= 3); cell edge = box/ncell must be >= rcut            */
+  float rcut;        /* cutoff radius rc (> 0); a pair contributes iff s < rc^2, strictly (R5)                */
+  float eps;         /* Plummer softening length (> 0); eps^2 is added to s in the Newtonian term only (R3)  */
+  float poly[6];     /* c0..c5 of the grid-force fit P(s), s = r^2 (R4); see srpp_default_poly               */
+} srpp_params;
+
+typedef struct srpp_ctx srpp_ctx;
+
+/* Counters of the last srpp_accel, for harness reporting (host memory). */
+typedef struct {
+  uint64_t work_items;      /* warp-level work items executed (target tile x source chunk)                  */
+  uint64_t pair_slots;      /* pair evaluations issued, padding included                                     */
+  uint64_t candidate_pairs; /* W = sum_c n_c * sum_{c' in 27-stencil(c)} n_c'             */
+  uint32_t max_cell_count;  /* largest cell occupancy                                                       */
+  uint32_t uniform_mass;    /* 1 if every particle carries the same mass (fast path taken)                   */
+} srpp_stats;
+
+/* The six default coefficients (degree-5 fit in s to a Gaussian-filtered point
+ * mass, sigma = 1.2, with P(9) = 1/27), written to poly_host[6]. */
+int32_t srpp_default_poly(float* poly_host);
+
+/* Bytes of device workspace needed for n particles with these parameters (256-byte aligned base).
+ * Holds: cell ids, radix-sort ping-pong keys/values and digit histograms, cell_start[ncells+1],
+ * perm[n], sorted float4[n], per-cell work tables, fp64 accumulators double[3n], flags/counters. */
+int32_t srpp_workspace_bytes(const srpp_params* params, int64_t n, size_t* bytes_host);
+
+/* Validates `params`, records workspace + stream.  The context is host memory owned by the library. */
+int32_t srpp_create(srpp_ctx** ctx, const srpp_params* params, void* workspace, size_t workspace_bytes,
+                    void* cuda_stream);
+void srpp_destroy(srpp_ctx* ctx);
+
+/*
+ * A1-A4: chaining mesh = stable counting sort of the particles by linear cell id.
+ *   cell coordinate per axis in fp32: inv = (float)ncell/box; c = min((int)floorf(x*inv), ncell-1) (R10)
+ *   cid = cx + ncx*(cy + ncy*cz) (R11); inside a cell, ascending original index (R12).
+ * pos_mass: device float4[n] (x, y, z, m), read-only, 0 <= x < L required (else SRPP_ERR_DOMAIN).
+ * Synchronises the stream once to read the error flag.  Results are bit-exact reproducible.
+ */
+int32_t srpp_build_mesh(srpp_ctx* ctx, const float* pos_mass, int64_t n);
+
+/* Borrowed device views into the workspace, valid until the next srpp_build_mesh / srpp_destroy:
+ *   cell_start uint32[ncells+1] (cell_start[ncells] = n), perm uint32[n] (perm[k] = original index of the
+ *   k-th particle in (cid, index) order), sorted float4[n] (sorted[k] = pos_mass[perm[k]]).
+ * Any of the three output pointers may be NULL. */
+int32_t srpp_get_mesh(const srpp_ctx* ctx, const uint32_t** cell_start, const uint32_t** perm,
+                      const float** sorted);
+
+/* A5-A6: short-range accelerations of all n particles from the last mesh, written in the caller's
+ * ORIGINAL particle order (R15) as float4 (ax, ay, az, 0).  fp32 pair arithmetic, MUFU rsqrt,
+ * per-item fp32 partial sums folded into fp64 accumulators.  Asynchronous on the stream. */
+int32_t srpp_accel(srpp_ctx* ctx, float* acc);
+
+/* Counters of the last srpp_accel (synchronises the stream). */
+int32_t srpp_get_stats(srpp_ctx* ctx, srpp_stats* stats_host);
+
+/* A7: sub-cycled kick, v <- fmaf(a, kdt, v) per component in fp32 (R16); .w lanes untouched.
+ * vel, acc: device float4[n].  Asynchronous. */
+int32_t srpp_kick(srpp_ctx* ctx, float* vel, const float* acc, float kdt, int64_t n);
+
+/* Stream (drift): x <- wrap(fmaf(v, dt, x)) per component in fp32, result in [0, L) (a value that rounds
+ * to L becomes 0; R13, R17).  Requires |v*dt| < L.  pos_mass is updated in place.  Asynchronous. */
+int32_t srpp_stream(srpp_ctx* ctx, float* pos_mass, const float* vel, float dt, int64_t n);
+
+/* End-to-end convenience for callers holding HOST arrays: copies pos_mass_host[4n] (and vel_host[4n] if
+ * not NULL) to the device, builds the mesh, computes accelerations, optionally kicks (vel_host != NULL:
+ * v <- v + kdt*a, copied back), copies acc back to acc_host[4n].  Device scratch for the particle arrays
+ * is taken from `device_scratch` (>= 48*n bytes, caller-owned device memory).  Synchronises. */
+int32_t srpp_step_host(srpp_ctx* ctx, const float* pos_mass_host, float* vel_host, float* acc_host,
+                       float kdt, int64_t n, void* device_scratch, size_t device_scratch_bytes);
+
+/* Static strings. */
+const char* srpp_strerror(int32_t status);
+const char* srpp_last_cuda_error(const srpp_ctx* ctx);
+int32_t srpp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SRPP_H_ */

@@ -1,0 +1,277 @@
+// srpp_api.cu -- the C ABI declared in include/srpp.h: argument validation, workspace carve-up,
+// host-side constants (fp64 re-expansion of the polynomial), and the calls into the kernels.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "srpp_internal.cuh"
+
+namespace srpp {
+
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// Carve the workspace; with ctx == nullptr only the size is computed.
+size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
+  const size_t nn = (size_t)(n > 0 ? n : 1);
+  const size_t ncells = (size_t)p.ncell[0] * p.ncell[1] * p.ncell[2];
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+  const size_t o_flags = take(sizeof(DevFlags));
+  const size_t o_k0 = take(4 * nn), o_k1 = take(4 * nn), o_v0 = take(4 * nn), o_v1 = take(4 * nn);
+  const size_t max_sort_blocks = 148 * 2 * kSortBlocksPerSM;   // generous upper bound on the sort grid
+  const size_t o_hist = take(4 * (size_t)kRadix * max_sort_blocks);
+  const size_t o_cs = take(4 * (ncells + 1));
+  const size_t o_sorted = take(16 * nn);
+  const size_t o_prefix = take(8 * (ncells + 1));
+  const size_t o_tmp = take(8 * ((ncells + 4095) / 4096 + 1));
+  const size_t o_acc = take(8 * 3 * nn);
+  if (c) {
+    char* b = c->ws;
+    c->flags = (DevFlags*)(b + o_flags);
+    c->keys[0] = (uint32_t*)(b + o_k0); c->keys[1] = (uint32_t*)(b + o_k1);
+    c->vals[0] = (uint32_t*)(b + o_v0); c->vals[1] = (uint32_t*)(b + o_v1);
+    c->hist = (uint32_t*)(b + o_hist);
+    c->cell_start = (uint32_t*)(b + o_cs);
+    c->sorted = (float4*)(b + o_sorted);
+    c->item_prefix = (unsigned long long*)(b + o_prefix);
+    c->scan_tmp = (unsigned long long*)(b + o_tmp);
+    c->acc64 = (double*)(b + o_acc);
+  }
+  return off;
+}
+
+static int32_t validate(const srpp_params* p) {
+  if (!p) return SRPP_ERR_INVALID_ARG;
+  for (int a = 0; a < 3; ++a)
+    if (!(p->box[a] > 0.f) || !isfinite(p->box[a])) return SRPP_ERR_INVALID_ARG;
+  if (!(p->rcut > 0.f) || !isfinite(p->rcut) || !(p->eps > 0.f) || !isfinite(p->eps)) return SRPP_ERR_INVALID_ARG;
+  for (int k = 0; k < 6; ++k)
+    if (!isfinite(p->poly[k])) return SRPP_ERR_INVALID_ARG;
+  int64_t ncells = 1;
+  for (int a = 0; a < 3; ++a) {
+    if (p->ncell[a] < 3) return SRPP_ERR_GEOMETRY;             // 27-cell stencil needs 3 distinct cells (R8)
+    if ((double)p->box[a] / (double)p->ncell[a] < (double)p->rcut) return SRPP_ERR_GEOMETRY;
+    ncells *= p->ncell[a];
+    if (ncells > (1 << 24)) return SRPP_ERR_GEOMETRY;
+  }
+  return SRPP_OK;
+}
+
+static int32_t cuda_fail(srpp_ctx* c, cudaError_t e) {
+  if (c) snprintf(c->cuda_err, sizeof(c->cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+  return SRPP_ERR_CUDA;
+}
+
+}  // namespace srpp
+
+using namespace srpp;
+
+extern "C" {
+
+int32_t srpp_version(void) { return SRPP_VERSION; }
+
+int32_t srpp_default_poly(float* poly_host) {
+  if (!poly_host) return SRPP_ERR_INVALID_ARG;
+  // SURVEY.md Appendix A (reading R4): fp32 bit patterns of the constrained least-squares fit
+  static const uint32_t bits[6] = {0x3EDEAD5Du, 0xBE36288Au, 0x3D2403BCu, 0xBBB0860Au, 0x39CFCFAAu, 0xB74AC976u};
+  memcpy(poly_host, bits, sizeof(bits));
+  return SRPP_OK;
+}
+
+int32_t srpp_workspace_bytes(const srpp_params* params, int64_t n, size_t* bytes_host) {
+  if (!bytes_host) return SRPP_ERR_INVALID_ARG;
+  const int32_t v = validate(params);
+  if (v != SRPP_OK) return v;
+  if (n < 0 || n >= ((int64_t)1 << 31)) return SRPP_ERR_INVALID_ARG;
+  *bytes_host = workspace_layout(*params, n, nullptr);
+  return SRPP_OK;
+}
+
+int32_t srpp_create(srpp_ctx** out, const srpp_params* params, void* workspace, size_t workspace_bytes,
+                    void* cuda_stream) {
+  if (!out) return SRPP_ERR_INVALID_ARG;
+  *out = nullptr;
+  const int32_t v = validate(params);
+  if (v != SRPP_OK) return v;
+  if (!workspace) return SRPP_ERR_INVALID_ARG;
+  if (((uintptr_t)workspace & 255u) != 0) return SRPP_ERR_WORKSPACE;
+  if (workspace_bytes < workspace_layout(*params, 0, nullptr)) return SRPP_ERR_WORKSPACE;
+  srpp_ctx* c = new (std::nothrow) srpp_ctx();
+  if (!c) return SRPP_ERR_INVALID_ARG;
+  memset(c, 0, sizeof(*c));
+  c->params = *params;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->ws = (char*)workspace;
+  c->ws_bytes = workspace_bytes;
+  c->n = -1;
+  cudaError_t e = cudaGetDevice(&c->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
+  if (e != cudaSuccess) { delete c; return SRPP_ERR_CUDA; }
+  c->force_blocks_per_sm = query_force_occupancy();
+
+  Geometry& g = c->geo;
+  int64_t ncells = 1;
+  for (int a = 0; a < 3; ++a) {
+    g.box[a] = params->box[a];
+    g.ncell[a] = params->ncell[a];
+    g.inv_cell[a] = (float)params->ncell[a] / params->box[a];   // one IEEE fp32 division (R10)
+    g.cell_w[a] = params->box[a] / (float)params->ncell[a];
+    ncells *= params->ncell[a];
+  }
+  g.ncells = (int32_t)ncells;
+  int bits = 1;
+  while (((int64_t)1 << bits) < ncells) ++bits;
+  c->sort_passes = (bits + kRadixBits - 1) / kRadixBits;
+
+  // force constants, in fp64: u = s + eps2 with eps2 the fp32 value the kernel adds, Q(u) = P(u - eps2)
+  const double e2 = (double)params->eps * (double)params->eps;
+  c->fc.eps2 = (float)e2;
+  const double e2f = (double)c->fc.eps2;
+  c->fc.rc2e = (float)((double)params->rcut * (double)params->rcut + e2f);
+  double q[6];
+  for (int k = 0; k < 6; ++k) {
+    double acc = 0.0, binom = 1.0, powr = 1.0;   // sum_{j>=k} c_j C(j,k) (-e2f)^(j-k)
+    for (int j = k; j < 6; ++j) {
+      acc += (double)params->poly[j] * binom * powr;
+      binom = binom * (double)(j + 1) / (double)(j + 1 - k);
+      powr *= -e2f;
+    }
+    q[k] = acc;
+  }
+  // Round -Q's coefficients to fp32.  Plain rounding leaves |Q~ - Q| up to ~4e-7 near the cutoff (the u^k
+  // amplify each half-ulp), where f itself is only ~1e-5, so pick, among the 3^6 neighbours within one ulp,
+  // the set that minimises max |Q~(u) - Q(u)| over the outer part of the range (where |f| is small).
+  float base[6], best[6];
+  for (int k = 0; k < 6; ++k) best[k] = base[k] = (float)(-q[k]);
+  const double u_hi = (double)c->fc.rc2e, u_lo = u_hi / 3.0;
+  double best_err = INFINITY;
+  for (int code = 0; code < 729; ++code) {
+    float cand[6];
+    int t = code;
+    for (int k = 0; k < 6; ++k, t /= 3) {
+      const int d = t % 3 - 1;
+      cand[k] = d == 0 ? base[k] : nextafterf(base[k], d > 0 ? INFINITY : -INFINITY);
+    }
+    double worst = 0.0;
+    for (int i = 0; i <= 64; ++i) {
+      const double u = u_lo + (u_hi - u_lo) * i / 64.0;
+      double e = 0.0;
+      for (int k = 5; k >= 0; --k) e = e * u + ((double)cand[k] + q[k]);
+      worst = fmax(worst, fabs(e));
+    }
+    if (worst < best_err) { best_err = worst; memcpy(best, cand, sizeof(best)); }
+  }
+  for (int k = 0; k < 6; ++k) c->fc.nq[k] = best[k];
+  *out = c;
+  return SRPP_OK;
+}
+
+void srpp_destroy(srpp_ctx* c) { delete c; }
+
+int32_t srpp_build_mesh(srpp_ctx* c, const float* pos_mass, int64_t n) {
+  if (!c || n < 0 || n >= ((int64_t)1 << 31) || (n > 0 && !pos_mass)) return SRPP_ERR_INVALID_ARG;
+  c->n = -1;
+  if (workspace_layout(c->params, n, nullptr) > c->ws_bytes) return SRPP_ERR_WORKSPACE;
+  workspace_layout(c->params, n, c);
+  cudaError_t e = launch_build_mesh(c, (const float4*)pos_mass, n);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  float m0 = 1.0f;
+  if (n > 0) e = cudaMemcpyAsync(&m0, pos_mass + 3, sizeof(float), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(&c->flags_host, c->flags, sizeof(DevFlags), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  if (c->flags_host.domain_error) return SRPP_ERR_DOMAIN;
+  c->uniform_mass = (c->flags_host.mass_nonuniform == 0);
+  c->mass0 = m0;
+  c->n = n;
+  return SRPP_OK;
+}
+
+int32_t srpp_get_mesh(const srpp_ctx* c, const uint32_t** cell_start, const uint32_t** perm, const float** sorted) {
+  if (!c) return SRPP_ERR_INVALID_ARG;
+  if (c->n < 0) return SRPP_ERR_STATE;
+  if (cell_start) *cell_start = c->cell_start;
+  if (perm) *perm = c->perm;
+  if (sorted) *sorted = (const float*)c->sorted;
+  return SRPP_OK;
+}
+
+int32_t srpp_accel(srpp_ctx* c, float* acc) {
+  if (!c) return SRPP_ERR_INVALID_ARG;
+  if (c->n < 0) return SRPP_ERR_STATE;
+  if (c->n > 0 && !acc) return SRPP_ERR_INVALID_ARG;
+  const cudaError_t e = launch_accel(c, (float4*)acc);
+  return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
+}
+
+int32_t srpp_get_stats(srpp_ctx* c, srpp_stats* s) {
+  if (!c || !s) return SRPP_ERR_INVALID_ARG;
+  if (c->n < 0) return SRPP_ERR_STATE;
+  cudaError_t e = cudaMemcpyAsync(&c->flags_host, c->flags, sizeof(DevFlags), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  s->work_items = c->flags_host.total_items;
+  s->pair_slots = c->flags_host.pair_slots;
+  s->candidate_pairs = c->flags_host.candidate_pairs;
+  s->max_cell_count = c->flags_host.max_cell_count;
+  s->uniform_mass = c->uniform_mass ? 1u : 0u;
+  return SRPP_OK;
+}
+
+int32_t srpp_kick(srpp_ctx* c, float* vel, const float* acc, float kdt, int64_t n) {
+  if (!c || n < 0 || (n > 0 && (!vel || !acc)) || !isfinite(kdt)) return SRPP_ERR_INVALID_ARG;
+  const cudaError_t e = launch_kick(c, (float4*)vel, (const float4*)acc, kdt, n);
+  return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
+}
+
+int32_t srpp_stream(srpp_ctx* c, float* pos_mass, const float* vel, float dt, int64_t n) {
+  if (!c || n < 0 || (n > 0 && (!pos_mass || !vel)) || !isfinite(dt)) return SRPP_ERR_INVALID_ARG;
+  const cudaError_t e = launch_stream(c, (float4*)pos_mass, (const float4*)vel, dt, n);
+  return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
+}
+
+int32_t srpp_step_host(srpp_ctx* c, const float* pos_mass_host, float* vel_host, float* acc_host, float kdt,
+                       int64_t n, void* device_scratch, size_t device_scratch_bytes) {
+  if (!c || n < 0 || (n > 0 && (!pos_mass_host || !acc_host || !device_scratch))) return SRPP_ERR_INVALID_ARG;
+  const size_t bytes = 16 * (size_t)n;
+  if (device_scratch_bytes < 3 * bytes || ((uintptr_t)device_scratch & 15u)) return SRPP_ERR_WORKSPACE;
+  float* d_pos = (float*)device_scratch;
+  float* d_acc = (float*)((char*)device_scratch + bytes);
+  float* d_vel = (float*)((char*)device_scratch + 2 * bytes);
+  cudaError_t e = cudaMemcpyAsync(d_pos, pos_mass_host, bytes, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess && vel_host) e = cudaMemcpyAsync(d_vel, vel_host, bytes, cudaMemcpyHostToDevice, c->stream);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  int32_t rc = srpp_build_mesh(c, d_pos, n);
+  if (rc != SRPP_OK) return rc;
+  rc = srpp_accel(c, d_acc);
+  if (rc != SRPP_OK) return rc;
+  if (vel_host) {
+    rc = srpp_kick(c, d_vel, d_acc, kdt, n);
+    if (rc != SRPP_OK) return rc;
+    e = cudaMemcpyAsync(vel_host, d_vel, bytes, cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+  }
+  e = cudaMemcpyAsync(acc_host, d_acc, bytes, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
+}
+
+const char* srpp_strerror(int32_t s) {
+  switch (s) {
+    case SRPP_OK: return "ok";
+    case SRPP_ERR_INVALID_ARG: return "invalid argument";
+    case SRPP_ERR_GEOMETRY: return "geometry: need ncell >= 3, box/ncell >= rcut, <= 2^24 cells";
+    case SRPP_ERR_DOMAIN: return "domain: a position is outside [0, L) or not finite";
+    case SRPP_ERR_WORKSPACE: return "workspace too small or misaligned";
+    case SRPP_ERR_STATE: return "state: no valid chaining mesh (call srpp_build_mesh first)";
+    case SRPP_ERR_CUDA: return "CUDA runtime error";
+    default: return "unknown status";
+  }
+}
+
+const char* srpp_last_cuda_error(const srpp_ctx* c) { return c ? c->cuda_err : ""; }
+
+}  // extern "C"

@@ -1,0 +1,453 @@
+// srpp_force.cu -- short-range PP force (A5), write-back (A6), kick (A7) and stream for sm_100a.
+//
+//   a_i = sum_{j, s_ij < rc^2} m_j d_ij [ (s_ij + eps^2)^(-3/2) - P(s_ij) ]          (
+//                                                                                    PAPER.md:63,65)
+// Design:
+//   * Work item = (cell c, tile of <= 32*T consecutive sorted targets of c, chunk of <= 1024 consecutive
+//     positions of c's 27-cell source stream).  Items of all cells form one global index space
+//     (exclusive prefix over cells); autonomous WARPS pull item indices from one atomic counter, so a
+//     cell holding 600 k particles becomes ~10^6 small items spread over the whole chip -- the on-chip
+//     analogue of the paper's block splitting for load balance.
+//   * Targets live in registers as PACKED PAIRS (float2 = two targets), sources are broadcast from a
+//     warp-private shared-memory tile stored duplicated (x,x,y,y | z,z | m,m) so that every arithmetic
+//     instruction of the pair loop is a Blackwell packed-fp32 op (FFMA2/FADD2/FMUL2): 16 packed FMA-pipe
+//     instructions per two pair interactions, leaving issue slots for MUFU.RSQ and the cutoff select.
+//   * Periodic images are applied when a source segment is staged (a per-segment shift), never per pair.
+//     Staged coordinates are relative to integer reference points, so the wrap is exact in fp32.
+//   * u = s + eps^2 comes straight out of the FMA chain (seeded with eps^2); the grid-force polynomial
+//     is re-expanded in u on the host in fp64 (Q(u) = P(u - eps^2)), negated, so f = fma(r^2, r, -Q(u)).
+//   * Each item accumulates in fp32 from zero over <= 1024 sources and is folded into fp64 accumulators
+//     with red.global.add.f64; A6 converts to fp32 and writes in the caller's original order (R15).
+#include <algorithm>
+
+#include "srpp_internal.cuh"
+
+namespace srpp {
+
+// ------------------------------------------------------------------------------ stencil segments --
+// The 27-cell stencil of cell (cx,cy,cz) as <= 18 runs that are contiguous in sorted order: 9 (dy,dz)
+// rows x {main x-run, wrapped x-run}.  shift = periodic image offset to ADD to a source coordinate.
+struct Segment {
+  uint32_t start, end;      // sorted-index range
+  int xlo, cy, cz;          // first cell of the run (for the reference point)
+  float shift[3];
+};
+
+__device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint32_t* __restrict__ cell_start, int cx,
+                                                   int cy, int cz, int seg) {
+  Segment s;
+  const int row = seg >> 1, sx = seg & 1;
+  const int dy = row % 3 - 1, dz = row / 3 - 1;
+  int y = cy + dy, z = cz + dz;
+  s.shift[0] = 0.f; s.shift[1] = 0.f; s.shift[2] = 0.f;
+  if (y < 0) { y += g.ncell[1]; s.shift[1] = -g.box[1]; } else if (y >= g.ncell[1]) { y -= g.ncell[1]; s.shift[1] = g.box[1]; }
+  if (z < 0) { z += g.ncell[2]; s.shift[2] = -g.box[2]; } else if (z >= g.ncell[2]) { z -= g.ncell[2]; s.shift[2] = g.box[2]; }
+  const int ncx = g.ncell[0];
+  int xlo, xhi;  // inclusive; xhi < xlo means empty
+  if (cx >= 1 && cx <= ncx - 2) {
+    if (sx == 0) { xlo = cx - 1; xhi = cx + 1; } else { xlo = 0; xhi = -1; }
+  } else if (cx == 0) {
+    if (sx == 0) { xlo = ncx - 1; xhi = ncx - 1; s.shift[0] = -g.box[0]; } else { xlo = 0; xhi = 1; }
+  } else {
+    if (sx == 0) { xlo = ncx - 2; xhi = ncx - 1; } else { xlo = 0; xhi = 0; s.shift[0] = g.box[0]; }
+  }
+  s.xlo = xlo; s.cy = y; s.cz = z;
+  if (xhi < xlo) { s.start = 0; s.end = 0; return s; }
+  const int rowbase = ncx * (y + g.ncell[1] * z);
+  s.start = __ldg(&cell_start[rowbase + xlo]);
+  s.end = __ldg(&cell_start[rowbase + xhi + 1]);
+  return s;
+}
+
+__device__ __forceinline__ int targets_per_lane(uint32_t n_c) { return n_c <= 64u ? 2 : 4; }
+
+// ------------------------------------------------------------------- plan: items per cell, W, max --
+__global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__ cell_start, Geometry g,
+                                                     unsigned long long* __restrict__ items, DevFlags* flags) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned long long w = 0, slots = 0;
+  uint32_t nmax = 0;
+  if (c < g.ncells) {
+    const uint32_t n_c = __ldg(&cell_start[c + 1]) - __ldg(&cell_start[c]);
+    unsigned long long it = 0;
+    if (n_c) {
+      const int cx = c % g.ncell[0], cy = (c / g.ncell[0]) % g.ncell[1], cz = c / (g.ncell[0] * g.ncell[1]);
+      unsigned long long S = 0;
+      for (int seg = 0; seg < kMaxSeg; ++seg) {
+        const Segment s = stencil_segment(g, cell_start, cx, cy, cz, seg);
+        S += s.end - s.start;
+      }
+      const int T = targets_per_lane(n_c);
+      const unsigned long long ntile = (n_c + 32u * T - 1) / (32u * T);
+      const unsigned long long nchunk = (S + kSrcChunk - 1) / kSrcChunk;
+      it = ntile * nchunk;
+      w = (unsigned long long)n_c * S;
+      slots = ntile * 32ull * T * ((S + 3ull) & ~3ull);
+      nmax = n_c;
+    }
+    items[c] = it;
+  }
+  // block reduction of the statistics
+  for (int o = 16; o; o >>= 1) {
+    w += __shfl_xor_sync(0xffffffffu, w, o);
+    slots += __shfl_xor_sync(0xffffffffu, slots, o);
+    nmax = max(nmax, __shfl_xor_sync(0xffffffffu, nmax, o));
+  }
+  if ((threadIdx.x & 31) == 0) {
+    if (w) atomicAdd(&flags->candidate_pairs, w);
+    if (slots) atomicAdd(&flags->pair_slots, slots);
+    if (nmax) atomicMax(&flags->max_cell_count, nmax);
+  }
+}
+
+// ------------------------------------------------------------------ 64-bit exclusive scan (3 kernels) --
+constexpr int kScanThreads = 1024;
+constexpr int kScanPerThread = 4;
+constexpr int kScanBlock = kScanThreads * kScanPerThread;
+
+__device__ __forceinline__ unsigned long long block_exclusive_scan(unsigned long long v, unsigned long long* total) {
+  __shared__ unsigned long long wsum[32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  unsigned long long x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned long long y = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += y;
+  }
+  __syncthreads();  // protect wsum reuse across calls
+  if (lane == 31) wsum[wid] = x;
+  __syncthreads();
+  if (wid == 0) {
+    unsigned long long w = wsum[lane];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned long long y = __shfl_up_sync(0xffffffffu, w, o);
+      if (lane >= o) w += y;
+    }
+    wsum[lane] = w;
+  }
+  __syncthreads();
+  if (total) *total = wsum[31];
+  return (wid ? wsum[wid - 1] : 0ull) + (x - v);
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const unsigned long long* __restrict__ in, int n,
+                                                               unsigned long long* __restrict__ block_sums) {
+  const int base = blockIdx.x * kScanBlock + threadIdx.x * kScanPerThread;
+  unsigned long long s = 0;
+#pragma unroll
+  for (int j = 0; j < kScanPerThread; ++j) s += (base + j < n) ? in[base + j] : 0ull;
+  unsigned long long tot;
+  block_exclusive_scan(s, &tot);
+  if (threadIdx.x == 0) block_sums[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_top(unsigned long long* __restrict__ block_sums, int nb,
+                                                            unsigned long long* __restrict__ total_out,
+                                                            unsigned long long* __restrict__ total_out2) {
+  const int base = threadIdx.x * kScanPerThread;
+  unsigned long long v[kScanPerThread], s = 0;
+#pragma unroll
+  for (int j = 0; j < kScanPerThread; ++j) { v[j] = (base + j < nb) ? block_sums[base + j] : 0ull; s += v[j]; }
+  unsigned long long tot;
+  unsigned long long ex = block_exclusive_scan(s, &tot);
+#pragma unroll
+  for (int j = 0; j < kScanPerThread; ++j) { if (base + j < nb) block_sums[base + j] = ex; ex += v[j]; }
+  if (threadIdx.x == 0) { *total_out = tot; *total_out2 = tot; }
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_apply(unsigned long long* __restrict__ data, int n,
+                                                              const unsigned long long* __restrict__ block_sums) {
+  const int base = blockIdx.x * kScanBlock + threadIdx.x * kScanPerThread;
+  unsigned long long v[kScanPerThread], s = 0;
+#pragma unroll
+  for (int j = 0; j < kScanPerThread; ++j) { v[j] = (base + j < n) ? data[base + j] : 0ull; s += v[j]; }
+  unsigned long long ex = block_exclusive_scan(s, nullptr) + block_sums[blockIdx.x];
+#pragma unroll
+  for (int j = 0; j < kScanPerThread; ++j) { if (base + j < n) data[base + j] = ex; ex += v[j]; }
+}
+
+// ------------------------------------------------------------------------------------ A5: PP force --
+__device__ __forceinline__ float rsqrt_approx(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));   // one MUFU.RSQ
+  return y;
+}
+
+__device__ __forceinline__ void red_add_f64(double* addr, double v) {
+  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(addr), "d"(v) : "memory");
+}
+
+struct __align__(16) WarpScratch {
+  float4 xy[kSrcTile];      // (x, x, y, y) of a staged source, relative to the item's reference point
+  float2 zz[kSrcTile];      // (z, z)
+  float2 mm[kSrcTile];      // (m, m)
+  uint32_t seg_start[kMaxSeg + 1];   // stream offset of each segment; [kMaxSeg] = S
+  uint32_t seg_base[kMaxSeg];        // sorted index of each segment's first particle
+  float seg_ref[kMaxSeg][3];         // integer-valued reference point R_s of the segment's cells
+  float seg_delta[kMaxSeg][3];       // R_s - R_t + periodic shift  (exact for integer box lengths)
+};
+
+// One work item for one warp.  TP = target pairs per lane (T = 2*TP targets per lane).
+template <int TP, bool kUniformMass>
+__device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __restrict__ sorted, const ForceConst& fc,
+                                             uint32_t tgt_begin, uint32_t tgt_end, const float ref_t[3],
+                                             uint32_t p0, uint32_t p1, double* __restrict__ acc64, int lane) {
+  // ---- targets: lane holds pairs (k, k+32) of each 64-block, negated and relative to R_t
+  float2 ntx[TP], nty[TP], ntz[TP], ax[TP], ay[TP], az[TP];
+#pragma unroll
+  for (int t = 0; t < TP; ++t) {
+    const uint32_t k0 = tgt_begin + t * 64 + lane, k1 = k0 + 32;
+    float4 a = make_float4(-1.0e3f, -1.0e3f, -1.0e3f, 0.f), b = a;
+    if (k0 < tgt_end) { a = __ldg(&sorted[k0]); a.x -= ref_t[0]; a.y -= ref_t[1]; a.z -= ref_t[2]; }
+    if (k1 < tgt_end) { b = __ldg(&sorted[k1]); b.x -= ref_t[0]; b.y -= ref_t[1]; b.z -= ref_t[2]; }
+    ntx[t] = make_float2(-a.x, -b.x);
+    nty[t] = make_float2(-a.y, -b.y);
+    ntz[t] = make_float2(-a.z, -b.z);
+    ax[t] = ay[t] = az[t] = make_float2(0.f, 0.f);
+  }
+  const float2 e2 = make_float2(fc.eps2, fc.eps2);
+  const float2 c5 = make_float2(fc.nq[5], fc.nq[5]), c4 = make_float2(fc.nq[4], fc.nq[4]);
+  const float2 c3 = make_float2(fc.nq[3], fc.nq[3]), c2 = make_float2(fc.nq[2], fc.nq[2]);
+  const float2 c1 = make_float2(fc.nq[1], fc.nq[1]), c0 = make_float2(fc.nq[0], fc.nq[0]);
+  const float rc2e = fc.rc2e;
+
+  int seg = 0;  // monotone per-lane segment cursor (stream positions only grow)
+  for (uint32_t tile = p0; tile < p1; tile += kSrcTile) {
+    // ---- stage up to kSrcTile stream positions into the warp-private tile
+    __syncwarp();
+#pragma unroll
+    for (int j = 0; j < kSrcTile / 32; ++j) {
+      const uint32_t p = tile + j * 32 + lane;
+      float4 xy = make_float4(1.0e3f, 1.0e3f, 1.0e3f, 1.0e3f);
+      float2 zz = make_float2(1.0e3f, 1.0e3f), mm = make_float2(0.f, 0.f);
+      if (p < p1) {
+        while (p >= ws.seg_start[seg + 1]) ++seg;
+        const float4 v = __ldg(&sorted[ws.seg_base[seg] + (p - ws.seg_start[seg])]);
+        const float x = (v.x - ws.seg_ref[seg][0]) + ws.seg_delta[seg][0];
+        const float y = (v.y - ws.seg_ref[seg][1]) + ws.seg_delta[seg][1];
+        const float z = (v.z - ws.seg_ref[seg][2]) + ws.seg_delta[seg][2];
+        xy = make_float4(x, x, y, y);
+        zz = make_float2(z, z);
+        mm = make_float2(v.w, v.w);
+      }
+      ws.xy[j * 32 + lane] = xy;
+      ws.zz[j * 32 + lane] = zz;
+      if (!kUniformMass) ws.mm[j * 32 + lane] = mm;
+    }
+    __syncwarp();
+    // ---- pair loop: every source of the tile against the lane's 2*TP targets
+    const int cnt = (int)min((uint32_t)kSrcTile, (p1 - tile + 3u) & ~3u);
+#pragma unroll 4
+    for (int j = 0; j < cnt; ++j) {
+      const float4 sxy = ws.xy[j];
+      const float2 sz = ws.zz[j];
+      const float2 sx = make_float2(sxy.x, sxy.y), sy = make_float2(sxy.z, sxy.w);
+      float2 sm;
+      if (!kUniformMass) sm = ws.mm[j];
+#pragma unroll
+      for (int t = 0; t < TP; ++t) {
+        const float2 dx = __fadd2_rn(sx, ntx[t]);
+        const float2 dy = __fadd2_rn(sy, nty[t]);
+        const float2 dz = __fadd2_rn(sz, ntz[t]);
+        float2 u = __ffma2_rn(dx, dx, e2);
+        u = __ffma2_rn(dy, dy, u);
+        u = __ffma2_rn(dz, dz, u);
+        const float2 r = make_float2(rsqrt_approx(u.x), rsqrt_approx(u.y));
+        const float2 r2 = __fmul2_rn(r, r);
+        float2 q = __ffma2_rn(c5, u, c4);
+        q = __ffma2_rn(q, u, c3);
+        q = __ffma2_rn(q, u, c2);
+        q = __ffma2_rn(q, u, c1);
+        q = __ffma2_rn(q, u, c0);
+        float2 f = __ffma2_rn(r2, r, q);          // r^3 - Q(u)
+        f.x = (u.x < rc2e) ? f.x : 0.f;           // strict cutoff (R5), plain truncation (R6)
+        f.y = (u.y < rc2e) ? f.y : 0.f;
+        if (!kUniformMass) f = __fmul2_rn(f, sm);
+        ax[t] = __ffma2_rn(f, dx, ax[t]);
+        ay[t] = __ffma2_rn(f, dy, ay[t]);
+        az[t] = __ffma2_rn(f, dz, az[t]);
+      }
+    }
+  }
+  // ---- fold the fp32 partial sums into the fp64 accumulators (sorted order)
+#pragma unroll
+  for (int t = 0; t < TP; ++t) {
+    const uint32_t k0 = tgt_begin + t * 64 + lane, k1 = k0 + 32;
+    if (k0 < tgt_end) {
+      red_add_f64(&acc64[3 * (size_t)k0 + 0], (double)ax[t].x);
+      red_add_f64(&acc64[3 * (size_t)k0 + 1], (double)ay[t].x);
+      red_add_f64(&acc64[3 * (size_t)k0 + 2], (double)az[t].x);
+    }
+    if (k1 < tgt_end) {
+      red_add_f64(&acc64[3 * (size_t)k1 + 0], (double)ax[t].y);
+      red_add_f64(&acc64[3 * (size_t)k1 + 1], (double)ay[t].y);
+      red_add_f64(&acc64[3 * (size_t)k1 + 2], (double)az[t].y);
+    }
+  }
+}
+
+template <bool kUniformMass>
+__global__ void __launch_bounds__(kForceThreads, 2)
+k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_start,
+           const unsigned long long* __restrict__ item_prefix, Geometry g, ForceConst fc, DevFlags* flags,
+           double* __restrict__ acc64) {
+  __shared__ WarpScratch scratch[kForceWarps];
+  const int lane = threadIdx.x & 31;
+  WarpScratch& ws = scratch[threadIdx.x >> 5];
+  const unsigned long long total = flags->total_items;
+
+  for (;;) {
+    unsigned long long idx = 0;
+    if (lane == 0) idx = atomicAdd(&flags->item_counter, 1ull);
+    idx = __shfl_sync(0xffffffffu, idx, 0);
+    if (idx >= total) break;
+
+    // ---- 32-ary search: largest c with item_prefix[c] <= idx  (item_prefix[ncells] = total > idx)
+    int lo = 0, hi = g.ncells;            // invariant: prefix[lo] <= idx < prefix[hi]
+    while (hi - lo > 1) {
+      const int step = (hi - lo + 31) / 32;
+      const int probe = lo + lane * step;
+      const bool le = (probe < hi) && (__ldg(&item_prefix[probe]) <= idx);
+      const uint32_t ballot = __ballot_sync(0xffffffffu, le);
+      const int k = __popc(ballot);       // >= 1 (probe == lo always qualifies); qualifying lanes form a prefix
+      const int nlo = lo + (k - 1) * step;
+      hi = min(hi, nlo + step);
+      lo = nlo;
+    }
+    const int c = lo;
+    const uint32_t local = (uint32_t)(idx - __ldg(&item_prefix[c]));
+    const uint32_t cs0 = __ldg(&cell_start[c]), cs1 = __ldg(&cell_start[c + 1]);
+    const uint32_t n_c = cs1 - cs0;
+    const int T = targets_per_lane(n_c);
+    const uint32_t ntile = (n_c + 32u * T - 1) / (32u * T);
+    const uint32_t tile = local % ntile, chunk = local / ntile;   // chunk-major: neighbours share sources
+    const int cx = c % g.ncell[0], cy = (c / g.ncell[0]) % g.ncell[1], cz = c / (g.ncell[0] * g.ncell[1]);
+
+    // ---- segment table of this cell's source stream (lanes 0..17), prefix by warp scan
+    float ref_t[3] = {floorf(cx * g.cell_w[0]), floorf(cy * g.cell_w[1]), floorf(cz * g.cell_w[2])};
+    uint32_t len = 0;
+    Segment s;
+    if (lane < kMaxSeg) {
+      s = stencil_segment(g, cell_start, cx, cy, cz, lane);
+      len = s.end - s.start;
+    }
+    uint32_t incl = len;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += y;
+    }
+    __syncwarp();
+    if (lane < kMaxSeg) {
+      ws.seg_start[lane] = incl - len;
+      ws.seg_base[lane] = s.start;
+      const float rs[3] = {floorf(s.xlo * g.cell_w[0]), floorf(s.cy * g.cell_w[1]), floorf(s.cz * g.cell_w[2])};
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        ws.seg_ref[lane][a] = rs[a];
+        ws.seg_delta[lane][a] = (float)(((double)rs[a] - (double)ref_t[a]) + (double)s.shift[a]);
+      }
+    }
+    const uint32_t S = __shfl_sync(0xffffffffu, incl, kMaxSeg - 1);
+    if (lane == 0) ws.seg_start[kMaxSeg] = S;
+    __syncwarp();
+
+    const uint32_t p0 = chunk * kSrcChunk, p1 = min(S, p0 + kSrcChunk);
+    const uint32_t tb = cs0 + tile * 32u * T, te = min(cs1, tb + 32u * T);
+    if (T == 2)
+      process_item<1, kUniformMass>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane);
+    else
+      process_item<2, kUniformMass>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane);
+  }
+}
+
+// --------------------------------------------------------------------------------- A6: write-back --
+__global__ void __launch_bounds__(256) k_write_back(const double* __restrict__ acc64, const uint32_t* __restrict__ perm,
+                                                     int64_t n, float scale, float4* __restrict__ acc) {
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+    const double s = (double)scale;
+    const float ax = (float)(acc64[3 * k + 0] * s), ay = (float)(acc64[3 * k + 1] * s), az = (float)(acc64[3 * k + 2] * s);
+    acc[__ldg(&perm[k])] = make_float4(ax, ay, az, 0.f);
+  }
+}
+
+// ----------------------------------------------------------------------------- A7: kick, and stream --
+__global__ void __launch_bounds__(256) k_kick(float4* __restrict__ vel, const float4* __restrict__ acc, float kdt, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    float4 v = vel[i];
+    const float4 a = __ldg(&acc[i]);
+    v.x = __fmaf_rn(a.x, kdt, v.x);
+    v.y = __fmaf_rn(a.y, kdt, v.y);
+    v.z = __fmaf_rn(a.z, kdt, v.z);
+    vel[i] = v;
+  }
+}
+
+__device__ __forceinline__ float wrap_coord(float y, float L) {
+  if (y >= L) y -= L;
+  else if (y < 0.f) y += L;
+  if (!(y < L)) y = 0.f;
+  return y;
+}
+
+__global__ void __launch_bounds__(256) k_stream(float4* __restrict__ pos, const float4* __restrict__ vel, float dt,
+                                                 float Lx, float Ly, float Lz, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    float4 p = pos[i];
+    const float4 v = __ldg(&vel[i]);
+    p.x = wrap_coord(__fmaf_rn(v.x, dt, p.x), Lx);
+    p.y = wrap_coord(__fmaf_rn(v.y, dt, p.y), Ly);
+    p.z = wrap_coord(__fmaf_rn(v.z, dt, p.z), Lz);
+    pos[i] = p;
+  }
+}
+
+// ------------------------------------------------------------------------------------ host launchers --
+int query_force_occupancy() {
+  int a = 0, b = 0;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k_pp_force<true>, kForceThreads, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_pp_force<false>, kForceThreads, 0);
+  const int m = a < b ? a : b;
+  return m < 1 ? 1 : m;
+}
+
+cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
+  cudaStream_t st = c->stream;
+  const int64_t n = c->n;
+  const int32_t ncells = c->geo.ncells;
+  cudaError_t e;
+  if (n == 0) return cudaSuccess;
+  // reset queue head + statistics (keep the binning flags)
+  if ((e = cudaMemsetAsync(&c->flags->max_cell_count, 0, sizeof(DevFlags) - offsetof(DevFlags, max_cell_count), st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(c->acc64, 0, sizeof(double) * 3 * (size_t)n, st)) != cudaSuccess) return e;
+  k_plan_items<<<(ncells + 255) / 256, 256, 0, st>>>(c->cell_start, c->geo, c->item_prefix, c->flags);
+  const int nb = (ncells + kScanBlock - 1) / kScanBlock;
+  k_scan_reduce<<<nb, kScanThreads, 0, st>>>(c->item_prefix, ncells, c->scan_tmp);
+  k_scan_top<<<1, kScanThreads, 0, st>>>(c->scan_tmp, nb, &c->flags->total_items, &c->item_prefix[ncells]);
+  k_scan_apply<<<nb, kScanThreads, 0, st>>>(c->item_prefix, ncells, c->scan_tmp);
+  const int grid = c->num_sms * c->force_blocks_per_sm;
+  if (c->uniform_mass)
+    k_pp_force<true><<<grid, kForceThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
+  else
+    k_pp_force<false><<<grid, kForceThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
+  const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
+  k_write_back<<<grid_ew, 256, 0, st>>>(c->acc64, c->perm, n, c->uniform_mass ? c->mass0 : 1.0f, acc);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_kick(srpp_ctx* c, float4* vel, const float4* acc, float kdt, int64_t n) {
+  if (n == 0) return cudaSuccess;
+  const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
+  k_kick<<<grid_ew, 256, 0, c->stream>>>(vel, acc, kdt, n);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_stream(srpp_ctx* c, float4* pos_mass, const float4* vel, float dt, int64_t n) {
+  if (n == 0) return cudaSuccess;
+  const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
+  k_stream<<<grid_ew, 256, 0, c->stream>>>(pos_mass, vel, dt, c->params.box[0], c->params.box[1], c->params.box[2], n);
+  return cudaGetLastError();
+}
+
+}  // namespace srpp
