@@ -1,0 +1,354 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the short-range PP hot path on B200 (contract: see the round prompt / DESIGN.md).
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+    srpp_build_mesh (A1-A4)  ->  srpp_accel (A5-A6)  ->  srpp_kick (A7)
+on the workload BASELINE.json's target is quoted on: configs[3], the clustered 2^25-particle per-node load
+(`--config 4`; configs are numbered 1..5 as in SURVEY.md).  Metric: candidate pair interactions per second,
+W / t_step with W = sum_c n_c * sum_{c' in 27-stencil(c)} n_c' (depends on the input only).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+N > 1 (torchrun): the path has no exchange step (BASELINE.json: one GPU, no sharding) -> N independent
+replicas of the same workload, barrier + max-over-ranks timing, value = N * K * W / t.
+`--impl reference` times the fp64 CPU oracle (oracle/), as it stands, on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1411_3396_b200 import workloads  # noqa: E402  (input generators only; no arithmetic of the method)
+
+METRIC = "short_range_pair_interactions_per_s"
+UNIT = "pairs/s"
+FLOP_PER_PAIR = 30.0          # 11 FMA x 2 + 4 add + 3 mul + 1 rsqrt
+FP32_LANES_PER_SM = 128       # SMs x 128 lanes x 2 flop x f_max
+BIN_BYTES_PER_PARTICLE = 52   # 16 read (ids) + 16 read + 16 write (sorted) + 4 write (perm)
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return json.load(fh), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+# --------------------------------------------------------------------------------------- clocks --
+class ClockSampler:
+    """Samples SM clock + throttle reasons of one GPU every 200 ms through NVML while the timed region runs."""
+
+    REASONS = (("sw_power_cap", 0x4), ("hw_slowdown", 0x8), ("sw_thermal_slowdown", 0x20),
+               ("hw_thermal_slowdown", 0x40), ("hw_power_brake", 0x80))
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.power = [], set(), []
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception as exc:  # NVML missing: report that, never invent clocks
+            self._nv = None
+            self.error = repr(exc)
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
+                mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)) if hasattr(
+                    nv, "nvmlDeviceGetCurrentClocksEventReasons") else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for name, bit in self.REASONS:
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+
+    def summary(self) -> dict:
+        if self._nv is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"]}
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples), "power_w_max": max(self.power) if self.power else None}
+
+
+# ------------------------------------------------------------------------------ CPU oracle legs --
+def _mesh_candidates(oracle, pos, w):
+    """Per-cell chaining-mesh candidate counts of the workload's own mesh (oracle's counting sort)."""
+    cs, perm, _ = oracle.build_mesh(pos, w.box, w.ncell)
+    nz, ny, nx = w.ncell[2], w.ncell[1], w.ncell[0]
+    cnt = np.diff(cs.astype(np.int64)).reshape(nz, ny, nx)
+    sten = sum(np.roll(cnt, (dz, dy, dx), axis=(0, 1, 2)) for dz in (-1, 0, 1) for dy in (-1, 0, 1) for dx in (-1, 0, 1))
+    return cs, perm, cnt, sten
+
+
+def _oracle_sample(oracle, pos, w, n_targets, seed):
+    """half uniform over particles, half drawn in proportion to candidate count (halo cores).
+    Returns (targets, chaining-mesh candidates of those targets)."""
+    rng = np.random.default_rng(seed)
+    cs, perm, cnt, sten = _mesh_candidates(oracle, pos, w)
+    w_cell = (cnt * sten).ravel().astype(np.float64)
+    nw = n_targets // 2
+    cells = rng.choice(w_cell.size, size=nw, p=w_cell / w_cell.sum())
+    k = cs[cells].astype(np.int64) + (rng.random(nw) * np.diff(cs)[cells]).astype(np.int64)
+    t = np.concatenate([rng.integers(0, pos.shape[0], n_targets - nw), perm[k].astype(np.int64)])
+    # candidates of target i in the WORKLOAD's mesh = stencil sum of its cell
+    cid = oracle.cell_ids(pos[t], w.box, w.ncell)
+    cand = sten.ravel()[cid].astype(np.int64)
+    return t, cand
+
+
+def oracle_rate(oracle, pos, w, budget_s: float, seed: int = 0):
+    """Marginal rate of the oracle in the bench's unit: (candidates_B - candidates_A) / (t_B - t_A) for two nested
+    target samples A < B, which removes the fixed cost of the oracle's own cell-list build (paid once per call and
+    amortised over all N targets in a full evaluation).  Sample B is sized from A's timing to fill `budget_s`."""
+    prm = oracle.make_params(w.box, w.rcut, w.eps)
+    t_all, cand_all = _oracle_sample(oracle, pos, w, 4096, seed)
+    order = np.random.default_rng(seed + 1).permutation(t_all.shape[0])
+    t_all, cand_all = t_all[order], cand_all[order]
+    n_a = 64
+    t0 = time.perf_counter()
+    oracle.accel(pos, prm, targets=t_all[:8])
+    t_fixed = time.perf_counter() - t0                       # ~ the cell-list build
+    t0 = time.perf_counter()
+    oracle.accel(pos, prm, targets=t_all[:n_a])
+    t_a = time.perf_counter() - t0
+    per_cand = max(t_a - t_fixed, 1e-4) / max(int(cand_all[:n_a].sum()), 1)
+    csum = np.cumsum(cand_all)
+    n_b = int(np.searchsorted(csum, budget_s / per_cand)) + 1
+    n_b = int(min(max(n_b, 2 * n_a), t_all.shape[0]))
+    t0 = time.perf_counter()
+    oracle.accel(pos, prm, targets=t_all[:n_b])
+    t_b = time.perf_counter() - t0
+    d_c = int(cand_all[:n_b].sum() - cand_all[:n_a].sum())
+    rate = d_c / max(t_b - t_a, 1e-9)
+    return {"value": rate, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "%s: %d targets (half uniform, half work-weighted; SURVEY.md 8(d)), %d chaining-mesh candidate "
+                      "pairs in %.1f s of fp64 oracle time; marginal rate between nested samples of %d and %d targets "
+                      "(fixed cell-list build of %.1f s per call excluded)"
+                      % (w.name, n_b, d_c, t_b - t_a, n_a, n_b, t_fixed)}
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle, as it stands, on the host cores; each step = one bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    pos = workloads.generate(w)
+    prm = oracle.make_params(w.box, w.rcut, w.eps)
+    t_all, cand_all = _oracle_sample(oracle, pos, w, 4096, 0)
+    order = np.random.default_rng(1).permutation(t_all.shape[0])
+    t_all, cand_all = t_all[order], cand_all[order]
+    total_budget = args.ref_budget
+    t0 = time.perf_counter()
+    oracle.accel(pos, prm, targets=t_all[:8])
+    t_fixed = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    oracle.accel(pos, prm, targets=t_all[:64])
+    t_a = time.perf_counter() - t0
+    per_cand = max(t_a - t_fixed, 1e-4) / max(int(cand_all[:64].sum()), 1)
+    per_step = max(total_budget / (args.steps + args.warmup) - t_fixed, 1.0)
+    n_s = int(min(max(int(np.searchsorted(np.cumsum(cand_all), per_step / per_cand)) + 1, 16), t_all.shape[0]))
+    tgt, cand = t_all[:n_s], int(cand_all[:n_s].sum())
+    for _ in range(args.warmup):
+        oracle.accel(pos, prm, targets=tgt)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.accel(pos, prm, targets=tgt)
+    dt = time.perf_counter() - t0
+    value = cand * args.steps / dt
+    sample = ("%s: each step = %d targets (half uniform, half work-weighted), %d chaining-mesh candidate pairs; the "
+              "oracle's own cell-list build (%.1f s per call) is inside every step" % (w.name, n_s, cand, t_fixed))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "n_particles": w.n, "sample_targets": n_s},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------- product arm --
+def run_product(args, w):
+    import torch
+    import torch.distributed as dist
+    from paper_1411_3396_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the srpp path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    binding.load()                                    # fail loudly if libsrpp.so is missing
+    pos = workloads.generate(w)                       # replicas: every rank runs the same workload
+    n = pos.shape[0]
+    sol = binding.Solver(w.box, w.ncell, w.rcut, w.eps, n_max=n, device=dev)
+    sol.set_timing(True)
+    d_pos = torch.from_numpy(pos).to(dev)
+    d_acc = torch.empty_like(d_pos)
+    d_vel = torch.zeros_like(d_pos)
+    kdt = w.dt if w.dt else 0.01
+
+    def step():
+        sol.build_mesh(d_pos)
+        sol.accel(d_acc)
+        sol.kick(d_vel, d_acc, kdt)
+
+    for _ in range(args.warmup):
+        step()
+    stats0 = sol.get_stats()
+    W = stats0["candidate_pairs"]
+    mesh_ms, accel_ms, force_ms = [], [], []
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local) as clocks:
+        ev0.record()
+        for _ in range(args.steps):
+            step()
+            if args.phase_timing:                      # reads events of this step (one extra stream sync per step)
+                t = sol.get_timings()
+                mesh_ms.append(t["mesh_ms"]); accel_ms.append(t["accel_ms"]); force_ms.append(t["force_ms"])
+        ev1.record()
+        barrier()
+    t_ms = max_over_ranks(ev0.elapsed_time(ev1))
+    stats1 = sol.get_stats()
+    launches = (stats1["kernel_launches"] - stats0["kernel_launches"])
+    value = world * args.steps * W / (t_ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    h_pos = torch.from_numpy(pos).pin_memory()
+    h_vel = torch.zeros((n, 4), dtype=torch.float32).pin_memory()
+    h_acc = torch.empty((n, 4), dtype=torch.float32).pin_memory()
+    scratch = torch.empty(48 * n, dtype=torch.uint8, device=dev)
+    sol.step_host(h_pos, h_vel, h_acc, kdt, scratch)            # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        sol.step_host(h_pos, h_vel, h_acc, kdt, scratch)        # synchronises: results are in host memory on return
+    barrier()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    e2e = {"value": world * args.e2e_steps * W / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 2 * 16 * n,
+           "d2h_bytes_per_step": 2 * 16 * n, "steps": args.e2e_steps, "ms_per_step": 1e3 * e2e_s / args.e2e_steps,
+           "api": "srpp_step_host (pinned host pos/vel in, acc/vel out)"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks, peak_kind = _peaks()
+    props = torch.cuda.get_device_properties(dev)
+    sms = props.multi_processor_count
+    clk = clocks.summary()
+    f_max_hz = 1e6 * float(peaks.get("sm_max_mhz") or clk.get("sm_max_mhz") or 1965.0)
+    peak_tflops = sms * FP32_LANES_PER_SM * 2 * f_max_hz / 1e12
+    force_avg_ms = float(np.mean(force_ms)) if force_ms else None
+    achieved = FLOP_PER_PAIR * W / (force_avg_ms * 1e-3) / 1e12 if force_avg_ms else None
+    probe = {"ffma_tflops": sol.probe_fp32(0, 4000) / 1e12, "ffma2_tflops": sol.probe_fp32(1, 4000) / 1e12}
+    ncells = w.ncell[0] * w.ncell[1] * w.ncell[2]
+    bin_bytes = BIN_BYTES_PER_PARTICLE * n + 8 * ncells
+    mesh_avg_ms = float(np.mean(mesh_ms)) if mesh_ms else None
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "baseline_config": "BASELINE.json configs[%d]" % (args.config - 1),
+                   "n_particles": n, "box": list(w.box), "ncell": list(w.ncell), "rcut": w.rcut, "eps": w.eps,
+                   "candidate_pairs_W": W, "max_cell_count": stats1["max_cell_count"],
+                   "step": "build_mesh + accel + kick", "parallelism": "replicas only (no exchange step)",
+                   "l2": "inputs larger than L2 (16 B x N = %d MiB per array)" % (16 * n >> 20)},
+        "clocks": clk, "e2e": e2e, "gpu_launches": launches,
+        "roofline": {"bound": "alu", "kernel": "k_pp_force", "achieved": achieved, "peak": peak_tflops,
+                     "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None, "traffic": None,
+                     "peak_kind": "nominal: %d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (sm_max_mhz, %s); "
+                                  "30 flop per candidate pair" % (sms, f_max_hz / 1e6, peak_kind),
+                     "launch_ms": force_avg_ms, "fp32_probe": probe,
+                     "frac_of_probe_ffma2": (achieved / probe["ffma2_tflops"]) if achieved else None},
+        "phases": {"mesh_ms": mesh_avg_ms, "accel_ms": float(np.mean(accel_ms)) if accel_ms else None,
+                   "force_ms": force_avg_ms,
+                   "accel_pairs_per_s": W / (np.mean(accel_ms) * 1e-3) if accel_ms else None,
+                   "binning_gbs": bin_bytes / (mesh_avg_ms * 1e-3) / 1e9 if mesh_avg_ms else None,
+                   "binning_frac_of_hbm": (bin_bytes / (mesh_avg_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]) if mesh_avg_ms else None,
+                   "hbm_gbs_peak": peaks["hbm_gbs"], "hbm_peak_kind": peak_kind},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle                                  # cpu_baseline leg: the one place the product arm may run it
+        oracle.build()
+        line["cpu_baseline"] = oracle_rate(oracle, pos, w, args.cpu_budget)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=sorted(workloads.CONFIGS))
+    ap.add_argument("--impl", default="srpp", choices=["srpp", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
+    ap.add_argument("--ref-budget", type=float, default=150.0, help="seconds for the whole --impl reference run")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-phase-timing", dest="phase_timing", action="store_false")
+    args = ap.parse_args()
+    w = workloads.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_product(args, w)
+
+
+if __name__ == "__main__":
+    main()

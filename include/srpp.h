@@ -67,7 +67,16 @@ typedef struct {
   uint64_t candidate_pairs; /* W = sum_c n_c * sum_{c' in 27-stencil(c)} n_c'             */
   uint32_t max_cell_count;  /* largest cell occupancy                                                       */
   uint32_t uniform_mass;    /* 1 if every particle carries the same mass (fast path taken)                   */
+  uint64_t kernel_launches; /* CUDA kernels this context has launched since srpp_create (all calls)          */
 } srpp_stats;
+
+/* Device times of the last srpp_build_mesh / srpp_accel, from CUDA events the library records on ITS
+ * stream around each phase when timing is enabled (milliseconds; -1 where no phase has run yet). */
+typedef struct {
+  float mesh_ms;   /* A1-A4: all binning kernels of the last srpp_build_mesh                                */
+  float accel_ms;  /* A5-A6: whole srpp_accel (work plan + PP force kernel + write-back)                     */
+  float force_ms;  /* A5 only: the PP force kernel launch                                                    */
+} srpp_timings;
 
 /* The six default coefficients (degree-5 fit in s to a Gaussian-filtered point
  * mass, sigma = 1.2, with P(9) = 1/27), written to poly_host[6]. */
@@ -106,6 +115,17 @@ int32_t srpp_accel(srpp_ctx* ctx, float* acc);
 
 /* Counters of the last srpp_accel (synchronises the stream). */
 int32_t srpp_get_stats(srpp_ctx* ctx, srpp_stats* stats_host);
+
+/* Enable (1) / disable (0) event recording around the phases; off by default.  srpp_get_timings
+ * synchronises the stream and reads the events of the last build/accel. */
+int32_t srpp_set_timing(srpp_ctx* ctx, int32_t enable);
+int32_t srpp_get_timings(srpp_ctx* ctx, srpp_timings* timings_host);
+
+/* FP32 peak probe for the "% of FP32 peak" report: runs a register-only FMA stream on
+ * every SM of the context's device and writes the sustained flop/s to *flops_per_s_host.
+ * variant 0 = scalar FFMA, 1 = packed FFMA2 (the pair loop's form); trips >= 1 scales the run time
+ * (trips = 2000 is about 10 ms).  Synchronises. */
+int32_t srpp_probe_fp32(srpp_ctx* ctx, int32_t variant, int32_t trips, double* flops_per_s_host);
 
 /* A7: sub-cycled kick, v <- fmaf(a, kdt, v) per component in fp32 (R16); .w lanes untouched.
  * vel, acc: device float4[n].  Asynchronous. */

@@ -19,7 +19,8 @@ STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "GEOMETRY", -3: "DOMAIN", -4: "W
 
 EXPORTS = ("srpp_version", "srpp_default_poly", "srpp_workspace_bytes", "srpp_create", "srpp_destroy",
            "srpp_build_mesh", "srpp_get_mesh", "srpp_accel", "srpp_get_stats", "srpp_kick", "srpp_stream",
-           "srpp_step_host", "srpp_strerror", "srpp_last_cuda_error")
+           "srpp_step_host", "srpp_strerror", "srpp_last_cuda_error", "srpp_set_timing", "srpp_get_timings",
+           "srpp_probe_fp32")
 
 
 class SrppParams(C.Structure):
@@ -29,7 +30,11 @@ class SrppParams(C.Structure):
 
 class SrppStats(C.Structure):
     _fields_ = [("work_items", C.c_uint64), ("pair_slots", C.c_uint64), ("candidate_pairs", C.c_uint64),
-                ("max_cell_count", C.c_uint32), ("uniform_mass", C.c_uint32)]
+                ("max_cell_count", C.c_uint32), ("uniform_mass", C.c_uint32), ("kernel_launches", C.c_uint64)]
+
+
+class SrppTimings(C.Structure):
+    _fields_ = [("mesh_ms", C.c_float), ("accel_ms", C.c_float), ("force_ms", C.c_float)]
 
 
 class SrppError(RuntimeError):
@@ -75,6 +80,12 @@ def load() -> C.CDLL:
     L.srpp_stream.argtypes = [vp, vp, vp, f32, i64]
     L.srpp_step_host.restype = i32
     L.srpp_step_host.argtypes = [vp, vp, vp, vp, f32, i64, vp, C.c_size_t]
+    L.srpp_set_timing.restype = i32
+    L.srpp_set_timing.argtypes = [vp, i32]
+    L.srpp_get_timings.restype = i32
+    L.srpp_get_timings.argtypes = [vp, C.POINTER(SrppTimings)]
+    L.srpp_probe_fp32.restype = i32
+    L.srpp_probe_fp32.argtypes = [vp, i32, i32, C.POINTER(C.c_double)]
     L.srpp_strerror.restype = C.c_char_p
     L.srpp_strerror.argtypes = [i32]
     L.srpp_last_cuda_error.restype = C.c_char_p
@@ -211,6 +222,21 @@ class Solver:
         s = SrppStats()
         self._check(self.lib.srpp_get_stats(self._ctx, C.byref(s)), "srpp_get_stats")
         return {k: int(getattr(s, k)) for k, _ in SrppStats._fields_}
+
+    def set_timing(self, enable: bool = True):
+        self._check(self.lib.srpp_set_timing(self._ctx, 1 if enable else 0), "srpp_set_timing")
+
+    def get_timings(self) -> dict:
+        """Device milliseconds of the last build_mesh / accel / force kernel (synchronises)."""
+        t = SrppTimings()
+        self._check(self.lib.srpp_get_timings(self._ctx, C.byref(t)), "srpp_get_timings")
+        return {k: float(getattr(t, k)) for k, _ in SrppTimings._fields_}
+
+    def probe_fp32(self, variant: int = 1, trips: int = 2000) -> float:
+        """Sustained FP32 flop/s of a register-only FMA stream (0 = FFMA, 1 = packed FFMA2)."""
+        out = C.c_double(0.0)
+        self._check(self.lib.srpp_probe_fp32(self._ctx, int(variant), int(trips), C.byref(out)), "srpp_probe_fp32")
+        return float(out.value)
 
     def kick(self, vel, acc, kdt: float):
         self._f4(vel, "vel"), self._f4(acc, "acc")

@@ -168,7 +168,49 @@ int32_t srpp_create(srpp_ctx** out, const srpp_params* params, void* workspace, 
   return SRPP_OK;
 }
 
-void srpp_destroy(srpp_ctx* c) { delete c; }
+void srpp_destroy(srpp_ctx* c) {
+  if (!c) return;
+  for (int i = 0; i < kNumEvents; ++i)
+    if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+  delete c;
+}
+
+int32_t srpp_set_timing(srpp_ctx* c, int32_t enable) {
+  if (!c) return SRPP_ERR_INVALID_ARG;
+  if (enable) {
+    for (int i = 0; i < kNumEvents; ++i)
+      if (!c->ev[i]) {
+        const cudaError_t e = cudaEventCreate(&c->ev[i]);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+      }
+  }
+  c->timing = enable != 0;
+  c->ev_mesh_valid = c->ev_accel_valid = false;
+  return SRPP_OK;
+}
+
+int32_t srpp_get_timings(srpp_ctx* c, srpp_timings* t) {
+  if (!c || !t) return SRPP_ERR_INVALID_ARG;
+  t->mesh_ms = t->accel_ms = t->force_ms = -1.0f;
+  if (!c->timing) return SRPP_ERR_STATE;
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  if (e == cudaSuccess && c->ev_mesh_valid) e = cudaEventElapsedTime(&t->mesh_ms, c->ev[kEvMesh0], c->ev[kEvMesh1]);
+  if (e == cudaSuccess && c->ev_accel_valid) {
+    e = cudaEventElapsedTime(&t->accel_ms, c->ev[kEvAccel0], c->ev[kEvAccel1]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&t->force_ms, c->ev[kEvForce0], c->ev[kEvForce1]);
+  }
+  return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
+}
+
+int32_t srpp_probe_fp32(srpp_ctx* c, int32_t variant, int32_t trips, double* flops_per_s_host) {
+  if (!c || !flops_per_s_host || variant < 0 || variant > 1 || trips < 1) return SRPP_ERR_INVALID_ARG;
+  // scratch word: the unused tail of the 256-byte flag block at the head of the workspace
+  static_assert(sizeof(DevFlags) <= 128, "flag block layout");
+  const cudaError_t e = run_fp32_probe(c->stream, variant, trips, flops_per_s_host, (float*)(c->ws + 128));
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  c->launches += 2;
+  return SRPP_OK;
+}
 
 int32_t srpp_build_mesh(srpp_ctx* c, const float* pos_mass, int64_t n) {
   if (!c || n < 0 || n >= ((int64_t)1 << 31) || (n > 0 && !pos_mass)) return SRPP_ERR_INVALID_ARG;
@@ -218,6 +260,7 @@ int32_t srpp_get_stats(srpp_ctx* c, srpp_stats* s) {
   s->candidate_pairs = c->flags_host.candidate_pairs;
   s->max_cell_count = c->flags_host.max_cell_count;
   s->uniform_mass = c->uniform_mass ? 1u : 0u;
+  s->kernel_launches = c->launches;
   return SRPP_OK;
 }
 

@@ -418,6 +418,7 @@ cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
   const int32_t ncells = c->geo.ncells;
   cudaError_t e;
   if (n == 0) return cudaSuccess;
+  if (c->timing) cudaEventRecord(c->ev[kEvAccel0], st);
   // reset queue head + statistics (keep the binning flags)
   if ((e = cudaMemsetAsync(&c->flags->max_cell_count, 0, sizeof(DevFlags) - offsetof(DevFlags, max_cell_count), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(c->acc64, 0, sizeof(double) * 3 * (size_t)n, st)) != cudaSuccess) return e;
@@ -427,12 +428,16 @@ cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
   k_scan_top<<<1, kScanThreads, 0, st>>>(c->scan_tmp, nb, &c->flags->total_items, &c->item_prefix[ncells]);
   k_scan_apply<<<nb, kScanThreads, 0, st>>>(c->item_prefix, ncells, c->scan_tmp);
   const int grid = c->num_sms * c->force_blocks_per_sm;
+  if (c->timing) cudaEventRecord(c->ev[kEvForce0], st);
   if (c->uniform_mass)
     k_pp_force<true><<<grid, kForceThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
   else
     k_pp_force<false><<<grid, kForceThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
+  if (c->timing) cudaEventRecord(c->ev[kEvForce1], st);
   const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
   k_write_back<<<grid_ew, 256, 0, st>>>(c->acc64, c->perm, n, c->uniform_mass ? c->mass0 : 1.0f, acc);
+  c->launches += 6;
+  if (c->timing) { cudaEventRecord(c->ev[kEvAccel1], st); c->ev_accel_valid = true; }
   return cudaGetLastError();
 }
 
@@ -440,6 +445,7 @@ cudaError_t launch_kick(srpp_ctx* c, float4* vel, const float4* acc, float kdt, 
   if (n == 0) return cudaSuccess;
   const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
   k_kick<<<grid_ew, 256, 0, c->stream>>>(vel, acc, kdt, n);
+  c->launches += 1;
   return cudaGetLastError();
 }
 
@@ -447,6 +453,7 @@ cudaError_t launch_stream(srpp_ctx* c, float4* pos_mass, const float4* vel, floa
   if (n == 0) return cudaSuccess;
   const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
   k_stream<<<grid_ew, 256, 0, c->stream>>>(pos_mass, vel, dt, c->params.box[0], c->params.box[1], c->params.box[2], n);
+  c->launches += 1;
   return cudaGetLastError();
 }
 

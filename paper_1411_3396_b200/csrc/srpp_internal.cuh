@@ -24,6 +24,9 @@ constexpr int kSrcTile = 128;                 // sources staged per warp-private
 constexpr int kSrcChunk = 1024;               // sources per work item (fp32 partial-sum length)
 constexpr int kMaxSeg = 18;                   // 9 (dy,dz) rows x up to 2 x-segments (periodic wrap)
 
+// timing events: mesh begin/end, accel begin, force-kernel begin/end, accel end
+enum { kEvMesh0 = 0, kEvMesh1, kEvAccel0, kEvForce0, kEvForce1, kEvAccel1, kNumEvents };
+
 // ---- device-side flag / counter block (first 256 bytes of the workspace) -------------------
 struct DevFlags {
   uint32_t domain_error;     // A1 found a position outside [0,L) or non-finite (R13)
@@ -82,6 +85,11 @@ struct srpp_ctx {
   const uint32_t* sorted_keys;
   srpp::DevFlags flags_host; // last read-back
   char cuda_err[256];
+  // optional per-phase device timing (srpp_set_timing): events recorded on `stream` around the phases
+  bool timing;
+  cudaEvent_t ev[srpp::kNumEvents];
+  bool ev_mesh_valid, ev_accel_valid;
+  uint64_t launches;         // kernels launched by this context so far (harness evidence)
 };
 
 namespace srpp {
@@ -95,5 +103,7 @@ cudaError_t launch_accel(srpp_ctx* c, float4* acc);
 cudaError_t launch_kick(srpp_ctx* c, float4* vel, const float4* acc, float kdt, int64_t n);
 cudaError_t launch_stream(srpp_ctx* c, float4* pos_mass, const float4* vel, float dt, int64_t n);
 int query_force_occupancy();
+// srpp_probe.cu
+cudaError_t run_fp32_probe(cudaStream_t st, int variant, int iters, double* flops_per_s, float* checksum);
 
 }  // namespace srpp

@@ -194,6 +194,7 @@ cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n) {
     c->sorted_keys = c->keys[0];
     return cudaMemsetAsync(c->cell_start, 0, sizeof(uint32_t) * ((size_t)ncells + 1), st);
   }
+  if (c->timing) cudaEventRecord(c->ev[kEvMesh0], st);
   const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
   k_cell_ids<<<grid_ew, 256, 0, st>>>(pos_mass, n, c->geo, c->keys[0], c->flags);
 
@@ -218,6 +219,8 @@ cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n) {
   c->perm = c->vals[c->sort_passes & 1];
   c->sorted_keys = c->keys[c->sort_passes & 1];
   k_finalize_mesh<<<grid_ew, 256, 0, st>>>(c->sorted_keys, c->perm, pos_mass, n, ncells, c->cell_start, c->sorted);
+  c->launches += 2 + 3 * (uint64_t)c->sort_passes;
+  if (c->timing) { cudaEventRecord(c->ev[kEvMesh1], st); c->ev_mesh_valid = true; }
   return cudaGetLastError();
 }
 
