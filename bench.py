@@ -204,30 +204,22 @@ def run_reference(args, w):
 # ----------------------------------------------------------------------------------- product arm --
 def run_product(args, w):
     import torch
-    import torch.distributed as dist
     from paper_1411_3396_b200 import binding
+    from paper_1411_3396_b200.replicas import Replicas
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the srpp path has no CPU fallback (use --impl reference for the oracle)")
+    local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+    rep = Replicas(backend="nccl", device=dev)        # replicas only: barrier + max-over-ranks, no data collective
+    world, rank = rep.world, rep.rank
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        rep.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    max_over_ranks = rep.max_over_ranks
 
     binding.load()                                    # fail loudly if libsrpp.so is missing
     pos = workloads.generate(w)                       # replicas: every rank runs the same workload
@@ -266,24 +258,25 @@ def run_product(args, w):
     value = world * args.steps * W / (t_ms * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
-    h_pos = torch.from_numpy(pos).pin_memory()
-    h_vel = torch.zeros((n, 4), dtype=torch.float32).pin_memory()
-    h_acc = torch.empty((n, 4), dtype=torch.float32).pin_memory()
-    scratch = torch.empty(48 * n, dtype=torch.uint8, device=dev)
-    sol.step_host(h_pos, h_vel, h_acc, kdt, scratch)            # warm-up
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.e2e_steps):
-        sol.step_host(h_pos, h_vel, h_acc, kdt, scratch)        # synchronises: results are in host memory on return
-    barrier()
-    e2e_s = max_over_ranks(time.perf_counter() - t0)
-    e2e = {"value": world * args.e2e_steps * W / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 2 * 16 * n,
-           "d2h_bytes_per_step": 2 * 16 * n, "steps": args.e2e_steps, "ms_per_step": 1e3 * e2e_s / args.e2e_steps,
-           "api": "srpp_step_host (pinned host pos/vel in, acc/vel out)"}
+    e2e = None
+    if args.e2e_steps > 0:
+        h_pos = torch.from_numpy(pos).pin_memory()
+        h_vel = torch.zeros((n, 4), dtype=torch.float32).pin_memory()
+        h_acc = torch.empty((n, 4), dtype=torch.float32).pin_memory()
+        scratch = torch.empty(48 * n, dtype=torch.uint8, device=dev)
+        sol.step_host(h_pos, h_vel, h_acc, kdt, scratch)            # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            sol.step_host(h_pos, h_vel, h_acc, kdt, scratch)        # synchronises: results are in host memory on return
+        barrier()
+        e2e_s = max_over_ranks(time.perf_counter() - t0)
+        e2e = {"value": world * args.e2e_steps * W / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 2 * 16 * n,
+               "d2h_bytes_per_step": 2 * 16 * n, "steps": args.e2e_steps, "ms_per_step": 1e3 * e2e_s / args.e2e_steps,
+               "api": "srpp_step_host (pinned host pos/vel in, acc/vel out)"}
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        rep.close()
         return
 
     peaks, peak_kind = _peaks()
@@ -326,8 +319,7 @@ def run_product(args, w):
         oracle.build()
         line["cpu_baseline"] = oracle_rate(oracle, pos, w, args.cpu_budget)
     print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    rep.close()
 
 
 def main():
