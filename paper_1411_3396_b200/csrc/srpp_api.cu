@@ -20,8 +20,10 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
   const size_t o_flags = take(sizeof(DevFlags));
   const size_t o_k0 = take(4 * nn), o_k1 = take(4 * nn), o_v0 = take(4 * nn), o_v1 = take(4 * nn);
-  const size_t max_sort_blocks = 148 * 2 * kSortBlocksPerSM;   // generous upper bound on the sort grid
-  const size_t o_hist = take(4 * (size_t)kRadix * max_sort_blocks);
+  int sp = 0, sb = 0;
+  plan_sort((int32_t)ncells, &sp, &sb);
+  const size_t o_hist = take(4 * ((size_t)1 << sb) * (nn / kSortTile + 1));   // [tiles][bins]
+  const size_t o_coltot = take(4 * (size_t)kSortMaxBins);
   const size_t o_cs = take(4 * (ncells + 1));
   const size_t o_sorted = take(16 * nn);
   const size_t o_prefix = take(8 * (ncells + 1));
@@ -32,12 +34,15 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
     c->flags = (DevFlags*)(b + o_flags);
     c->keys[0] = (uint32_t*)(b + o_k0); c->keys[1] = (uint32_t*)(b + o_k1);
     c->vals[0] = (uint32_t*)(b + o_v0); c->vals[1] = (uint32_t*)(b + o_v1);
+    c->keys_raw = c->keys[1];
     c->hist = (uint32_t*)(b + o_hist);
+    c->coltot = (uint32_t*)(b + o_coltot);
     c->cell_start = (uint32_t*)(b + o_cs);
     c->sorted = (float4*)(b + o_sorted);
     c->item_prefix = (unsigned long long*)(b + o_prefix);
     c->scan_tmp = (unsigned long long*)(b + o_tmp);
     c->acc64 = (double*)(b + o_acc);
+    c->pos_tmp = (float4*)(b + o_acc);
   }
   return off;
 }
@@ -121,9 +126,7 @@ int32_t srpp_create(srpp_ctx** out, const srpp_params* params, void* workspace, 
     ncells *= params->ncell[a];
   }
   g.ncells = (int32_t)ncells;
-  int bits = 1;
-  while (((int64_t)1 << bits) < ncells) ++bits;
-  c->sort_passes = (bits + kRadixBits - 1) / kRadixBits;
+  plan_sort(g.ncells, &c->sort_passes, &c->sort_digit_bits);
 
   // force constants, in fp64: u = s + eps2 with eps2 the fp32 value the kernel adds, Q(u) = P(u - eps2)
   const double e2 = (double)params->eps * (double)params->eps;

@@ -11,12 +11,14 @@
 namespace srpp {
 
 // ---- tunables ------------------------------------------------------------------------------
-constexpr int kRadixBits = 8;                 // LSD radix digit width (A2-A4 as digit-wise counting sort)
-constexpr int kRadix = 1 << kRadixBits;
-constexpr int kSortThreads = 256;             // 8 warps
-constexpr int kSortKeysPerThread = 8;         // warp handles 8 steps of 32 consecutive keys
-constexpr int kSortTile = kSortThreads * kSortKeysPerThread;  // 2048 keys per tile
-constexpr int kSortBlocksPerSM = 4;
+// binning: LSD counting sort of the cell id in wide digits, payload carried (srpp_mesh.cu)
+constexpr int kSortThreads = 512;             // 16 warps
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortItems = 8;                 // a warp handles 8 steps of 32 consecutive elements
+constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 elements per tile
+constexpr int kSortMinDigitBits = 5;          // >= 32 bins (one warp-row of the column scan)
+constexpr int kSortMaxDigitBits = 11;         // <= 2048 bins: two passes cover 2^22 cells
+constexpr int kSortMaxBins = 1 << kSortMaxDigitBits;
 
 constexpr int kForceThreads = 256;            // 8 autonomous warps per CTA
 constexpr int kForceWarps = kForceThreads / 32;
@@ -65,8 +67,11 @@ struct srpp_ctx {
   int force_blocks_per_sm;
   int64_t n_capacity;        // particles the workspace was sized for (== n of build_mesh)
   int64_t n;                 // particles of the last successful build_mesh, -1 before
-  int sort_passes;
+  int sort_passes;           // digits of the cell id (LSD passes)
+  int sort_digit_bits;       // bits per digit
   int sort_blocks;
+  int sort_blocks_per_sm;
+  bool sort_attr_set;
   bool uniform_mass;
   float mass0;
   // workspace carve-up (device pointers)
@@ -75,13 +80,16 @@ struct srpp_ctx {
   srpp::DevFlags* flags;
   uint32_t* keys[2];
   uint32_t* vals[2];
-  uint32_t* hist;            // [kRadix][sort_blocks]
+  uint32_t* keys_raw;        // cell ids in input order (aliases keys[1]: dead before pass 1 writes it)
+  uint32_t* hist;            // [tiles][nbins] per-tile digit histogram, scanned over tiles in place
+  uint32_t* coltot;          // [nbins] digit totals
+  float4* pos_tmp;           // payload ping-pong buffer (aliases acc64: mesh build and accel never overlap)
   uint32_t* cell_start;      // [ncells+1]
   float4* sorted;            // [n]
   unsigned long long* item_prefix;  // [ncells+1] exclusive prefix of per-cell work items
   unsigned long long* scan_tmp;     // block sums for the 64-bit scan
   double* acc64;             // [3n] fp64 accumulators, sorted order
-  const uint32_t* perm;      // == vals[sort_passes & 1]
+  const uint32_t* perm;      // == vals[(sort_passes - 1) & 1]
   const uint32_t* sorted_keys;
   srpp::DevFlags flags_host; // last read-back
   char cuda_err[256];
@@ -98,6 +106,7 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* ctx /*nullabl
 
 // srpp_mesh.cu
 cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n);
+void plan_sort(int32_t ncells, int* passes, int* digit_bits);
 // srpp_force.cu
 cudaError_t launch_accel(srpp_ctx* c, float4* acc);
 cudaError_t launch_kick(srpp_ctx* c, float4* vel, const float4* acc, float kdt, int64_t n);

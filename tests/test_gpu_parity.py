@@ -91,18 +91,27 @@ def test_binning_p8_example(oracle_mod, gpu):
             assert cs[cell] == 0 and cs[cell + 1] == 1
 
 
-@pytest.mark.parametrize("n", [0, 1, 2, 31, 33, 2047, 2049, 100003, 1500000])
+@pytest.mark.parametrize("n", [0, 1, 2, 31, 33, 2047, 2049, 4095, 4096, 4097, 8193, 100003, 1500000])
 def test_binning_uniform_ragged_sizes(oracle_mod, gpu, n):
     rng = np.random.default_rng(n + 1)
-    box, ncell = (41.6, 32.0, 64.0), (13, 10, 20)      # 2600 cells -> 2 radix passes
+    box, ncell = (41.6, 32.0, 64.0), (13, 10, 20)      # 2600 cells -> 12 bits -> 2 digits of 6 bits
     pos = np.ones((n, 4), dtype=np.float32)
     pos[:, :3] = (rng.random((n, 3)) * np.asarray(box)).astype(np.float32)
     pos[:, :3] = np.minimum(pos[:, :3], np.nextafter(np.asarray(box, dtype=np.float32), 0))
     _check_mesh(oracle_mod, gpu, pos, box, ncell)
 
 
-def test_binning_three_radix_passes_clustered(oracle_mod, gpu):
-    """> 65536 cells (3 digit passes), heavy cells, empty cells, random memory order."""
+@pytest.mark.parametrize("ncell,n", [((160, 160, 160), 300000),     # 4,096,000 cells: 22 bits -> 2 digits of 11
+                                     ((200, 170, 190), 200000),     # 6,460,000 cells: 23 bits -> 3 digits of 8
+                                     ((3, 3, 3), 5000)])            # 27 cells: one digit of 5 bits
+def test_binning_digit_plans(oracle_mod, gpu, ncell, n):
+    """Every digit plan of the LSD counting sort (1, 2 and 3 passes; 32 ... 2048 bins), clustered input."""
+    pos, box = workloads.scaled_clustered(n, ncell, seed=5, frac_halo=0.7, n_halo=30, a_range=(0.2, 2.0))
+    _check_mesh(oracle_mod, gpu, pos, box, ncell)
+
+
+def test_binning_two_digits_clustered(oracle_mod, gpu):
+    """84,480 cells (two 9-bit digits), heavy cells, empty cells, random memory order."""
     ncell = (48, 40, 44)
     pos, box = workloads.scaled_clustered(600000, ncell, seed=21, frac_halo=0.8, n_halo=40, a_range=(0.2, 2.0))
     sol = _check_mesh(oracle_mod, gpu, pos, box, ncell)
