@@ -24,6 +24,7 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   plan_sort((int32_t)ncells, &sp, &sb);
   const size_t o_hist = take(4 * ((size_t)1 << sb) * (nn / kSortTile + 1));   // [tiles][bins]
   const size_t o_coltot = take(4 * (size_t)kSortMaxBins);
+  const size_t o_colpart = take(4 * (size_t)kSortMaxBins * 16);
   const size_t o_cs = take(4 * (ncells + 1));
   const size_t o_sorted = take(16 * nn);
   const size_t o_prefix = take(8 * (ncells + 1));
@@ -37,6 +38,7 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
     c->keys_raw = c->keys[1];
     c->hist = (uint32_t*)(b + o_hist);
     c->coltot = (uint32_t*)(b + o_coltot);
+    c->colpart = (uint32_t*)(b + o_colpart);
     c->cell_start = (uint32_t*)(b + o_cs);
     c->sorted = (float4*)(b + o_sorted);
     c->item_prefix = (unsigned long long*)(b + o_prefix);

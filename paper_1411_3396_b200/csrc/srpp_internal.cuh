@@ -17,7 +17,7 @@ constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortItems = 8;                 // a warp handles 8 steps of 32 consecutive elements
 constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 elements per tile
 constexpr int kSortMinDigitBits = 5;          // >= 32 bins (one warp-row of the column scan)
-constexpr int kSortMaxDigitBits = 11;         // <= 2048 bins: two passes cover 2^22 cells
+constexpr int kSortMaxDigitBits = 10;         // <= 1024 bins (>= 4 elements per bin and tile): two passes cover 2^20 cells
 constexpr int kSortMaxBins = 1 << kSortMaxDigitBits;
 
 constexpr int kForceThreads = 256;            // 8 autonomous warps per CTA
@@ -83,6 +83,7 @@ struct srpp_ctx {
   uint32_t* keys_raw;        // cell ids in input order (aliases keys[1]: dead before pass 1 writes it)
   uint32_t* hist;            // [tiles][nbins] per-tile digit histogram, scanned over tiles in place
   uint32_t* coltot;          // [nbins] digit totals
+  uint32_t* colpart;         // [slices][nbins] slice totals of the column scan
   float4* pos_tmp;           // payload ping-pong buffer (aliases acc64: mesh build and accel never overlap)
   uint32_t* cell_start;      // [ncells+1]
   float4* sorted;            // [n]

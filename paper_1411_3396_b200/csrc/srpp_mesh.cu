@@ -4,7 +4,7 @@
 //   A1  cell id per particle, fp32:  c = min((int)floorf(x * inv), ncell-1), inv = (float)ncell/box
 //   A2-A4 histogram / exclusive scan / stable scatter.  A cell id has up to 24 bits and single cells hold
 //        millions of particles, so the counting sort is applied digit-wise, least significant digit first,
-//        with WIDE digits (<= 11 bits: two passes cover 2^22 cells) and with the particle PAYLOAD
+//        with WIDE digits (<= 10 bits: two passes cover 2^20 cells, three 2^24) and with the particle PAYLOAD
 //        (float4 position+mass and original index) carried through every pass.  All global traffic is
 //        streaming: each pass reads its input once, coalesced, re-orders a 4096-element tile by digit in
 //        shared memory, and writes per-digit runs.  No random gather remains (the first version sorted
@@ -13,7 +13,7 @@
 //        decides an output position: perm is bit-exact reproducible and equals the oracle's stable
 //        counting sort.
 //   cell_start = run boundaries of the sorted ids (= exclusive prefix sum of the cell histogram).
-// Per pass: [per-block digit histogram (fused into A1 for the first pass)] -> column scan over blocks ->
+// Per pass: [per-tile digit histogram (fused into A1 for the first pass)] -> column scan over tiles ->
 // scatter.  Algorithmic bytes per build: 52*N + 8*ncells; moved by this design for two
 // passes: 20 + 44 + 4 + 48 + 4 = 120 bytes per particle, all coalesced.
 // Paper context: PAPER.md:63/65 (direct PP short-range solver inside the hand-over radius); the chaining
@@ -154,29 +154,62 @@ __global__ void __launch_bounds__(kSortThreads) k_digit_hist(const uint32_t* __r
 }
 
 // -------------------------------------------- A3: per-digit exclusive scan over tiles + digit totals --
-// hist[tile][bin] -> exclusive prefix over tiles (in place); coltot[bin] = total of the bin.  One CTA
-// per 32 bins; warp w owns a slice of the tiles, lane = bin, so every access is a 128-byte row segment.
-__global__ void __launch_bounds__(1024) k_col_scan(uint32_t* __restrict__ hist, int64_t nblocks, int nbins,
-                                                    uint32_t* __restrict__ coltot) {
-  __shared__ uint32_t part[32][33];
+// hist[tile][bin] -> exclusive prefix over tiles (in place); coltot[bin] = total of the bin.  The tiles are
+// cut into kScanSlices slices; grid = (bins/32, slices); a CTA owns 32 bins x one slice, warp w a sub-slice,
+// lane = bin, so every access is a 128-byte row segment.  Phase 1 writes the slice totals, phase 2 adds the
+// totals of the earlier slices and rewrites its slice as exclusive prefixes.
+constexpr int kScanSlices = 8;
+
+__global__ void __launch_bounds__(1024) k_col_sum(const uint32_t* __restrict__ hist, int64_t ntiles, int nbins,
+                                                   uint32_t* __restrict__ part /*[kScanSlices][nbins]*/) {
+  __shared__ uint32_t sm[32][33];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int bin = blockIdx.x * 32 + lane;
-  const int64_t per = (nblocks + 31) / 32;
-  const int64_t b0 = min(nblocks, w * per), b1 = min(nblocks, b0 + per);
+  const int64_t per_slice = (ntiles + kScanSlices - 1) / kScanSlices;
+  const int64_t s0 = min(ntiles, blockIdx.y * per_slice), s1 = min(ntiles, s0 + per_slice);
+  const int64_t per = (s1 - s0 + 31) / 32;
+  const int64_t b0 = min(s1, s0 + w * per), b1 = min(s1, b0 + per);
+  uint32_t s = 0;
+#pragma unroll 8
+  for (int64_t b = b0; b < b1; ++b) s += __ldg(&hist[(size_t)b * nbins + bin]);
+  sm[w][lane] = s;
+  __syncthreads();
+  if (w == 0) {
+    uint32_t tot = 0;
+#pragma unroll
+    for (int ww = 0; ww < 32; ++ww) tot += sm[ww][lane];
+    part[(size_t)blockIdx.y * nbins + bin] = tot;
+  }
+}
+
+__global__ void __launch_bounds__(1024) k_col_scan(uint32_t* __restrict__ hist, int64_t ntiles, int nbins,
+                                                    const uint32_t* __restrict__ part, uint32_t* __restrict__ coltot) {
+  __shared__ uint32_t sm[32][33];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int bin = blockIdx.x * 32 + lane;
+  const int64_t per_slice = (ntiles + kScanSlices - 1) / kScanSlices;
+  const int64_t s0 = min(ntiles, blockIdx.y * per_slice), s1 = min(ntiles, s0 + per_slice);
+  const int64_t per = (s1 - s0 + 31) / 32;
+  const int64_t b0 = min(s1, s0 + w * per), b1 = min(s1, b0 + per);
   uint32_t s = 0;
 #pragma unroll 8
   for (int64_t b = b0; b < b1; ++b) s += hist[(size_t)b * nbins + bin];
-  part[w][lane] = s;
+  sm[w][lane] = s;
   __syncthreads();
-  uint32_t run = 0;
-  for (int ww = 0; ww < w; ++ww) run += part[ww][lane];
+  uint32_t run = 0, total = 0;
+  for (int y = 0; y < kScanSlices; ++y) {
+    const uint32_t v = __ldg(&part[(size_t)y * nbins + bin]);
+    if (y < (int)blockIdx.y) run += v;
+    total += v;
+  }
+  for (int ww = 0; ww < w; ++ww) run += sm[ww][lane];
 #pragma unroll 8
   for (int64_t b = b0; b < b1; ++b) {
     const uint32_t v = hist[(size_t)b * nbins + bin];
     hist[(size_t)b * nbins + bin] = run;
     run += v;
   }
-  if (w == 31) coltot[bin] = run;
+  if (blockIdx.y == 0 && w == 0) coltot[bin] = total;
 }
 
 // ---------------------------------------------------------------------- A4: stable scatter of a digit --
@@ -373,18 +406,34 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_digit_scatter(
 // --------------------------------------------------------------- cell_start from run boundaries --
 __global__ void __launch_bounds__(256) k_cell_start(const uint32_t* __restrict__ sorted_keys, int64_t n, int32_t ncells,
                                                      uint32_t* __restrict__ cell_start) {
-  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
-    const uint32_t key = __ldg(&sorted_keys[k]);
-    const int64_t prev = k > 0 ? (int64_t)__ldg(&sorted_keys[k - 1]) : -1;
-    // cells (prev, key] start at k: the first is `key` itself, the rest are empty cells before it
-    for (int64_t c = prev + 1; c <= (int64_t)key; ++c) cell_start[c] = (uint32_t)k;
-    if (k == n - 1)
-      for (int64_t c = (int64_t)key + 1; c <= (int64_t)ncells; ++c) cell_start[c] = (uint32_t)n;
+  constexpr int U = 8;
+  for (int64_t k0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * U; k0 < n; k0 += (int64_t)gridDim.x * blockDim.x * U) {
+    // keys k0-1 .. k0+U-1 (k0 is a multiple of 8: two 16-byte loads + the predecessor)
+    uint32_t key[U + 1];
+    key[0] = k0 > 0 ? __ldg(&sorted_keys[k0 - 1]) : 0u;
+    if (k0 + U <= n) {
+      const uint4 a = __ldg((const uint4*)&sorted_keys[k0]), b = __ldg((const uint4*)&sorted_keys[k0 + 4]);
+      key[1] = a.x; key[2] = a.y; key[3] = a.z; key[4] = a.w; key[5] = b.x; key[6] = b.y; key[7] = b.z; key[8] = b.w;
+    } else {
+#pragma unroll
+      for (int u = 0; u < U; ++u) key[u + 1] = k0 + u < n ? __ldg(&sorted_keys[k0 + u]) : 0u;
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t k = k0 + u;
+      if (k < n) {
+        const int64_t prev = k > 0 ? (int64_t)key[u] : -1;
+        // cells (prev, key] start at k: the first is `key` itself, the rest are empty cells before it
+        for (int64_t c = prev + 1; c <= (int64_t)key[u + 1]; ++c) cell_start[c] = (uint32_t)k;
+        if (k == n - 1)
+          for (int64_t c = (int64_t)key[u + 1] + 1; c <= (int64_t)ncells; ++c) cell_start[c] = (uint32_t)n;
+      }
+    }
   }
 }
 
 // ------------------------------------------------------------------------------------ host launcher --
-// Digit plan: the cell id has `bits` significant bits; passes = ceil(bits / 11), digits of equal width.
+// Digit plan: the cell id has `bits` significant bits; passes = ceil(bits / 10), digits of equal width.
 void plan_sort(int32_t ncells, int* passes, int* digit_bits) {
   int bits = kSortMinDigitBits;
   while (((int64_t)1 << bits) < (int64_t)ncells) ++bits;
@@ -433,16 +482,17 @@ cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n) {
     const int shift = p * dbits;
     const int o = p & 1;
     if (p > 0) k_digit_hist<<<hblocks, kSortThreads, smem_hist, st>>>(kin, n, shift, nbins, c->hist, tiles);
-    k_col_scan<<<nbins / 32, 1024, 0, st>>>(c->hist, tiles, nbins, c->coltot);
+    k_col_sum<<<dim3(nbins / 32, kScanSlices), 1024, 0, st>>>(c->hist, tiles, nbins, c->colpart);
+    k_col_scan<<<dim3(nbins / 32, kScanSlices), 1024, 0, st>>>(c->hist, tiles, nbins, c->colpart, c->coltot);
     if (p == 0)
       k_digit_scatter<true><<<blocks, kSortThreads, smem_scatter, st>>>(kin, pin, iin, c->keys[o], posbuf[o], c->vals[o], n, shift, nbins, c->hist, c->coltot, tiles);
     else
       k_digit_scatter<false><<<blocks, kSortThreads, smem_scatter, st>>>(kin, pin, iin, c->keys[o], posbuf[o], c->vals[o], n, shift, nbins, c->hist, c->coltot, tiles);
     kin = c->keys[o]; pin = posbuf[o]; iin = c->vals[o];
   }
-  const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
+  const int grid_ew = (int)std::min<int64_t>((n + 2047) / 2048, (int64_t)c->num_sms * 8);
   k_cell_start<<<grid_ew, 256, 0, st>>>(c->sorted_keys, n, ncells, c->cell_start);
-  c->launches += 2 + 3 * (uint64_t)passes - 1;
+  c->launches += 1 + 4 * (uint64_t)passes;
   if (c->timing) { cudaEventRecord(c->ev[kEvMesh1], st); c->ev_mesh_valid = true; }
   return cudaGetLastError();
 }

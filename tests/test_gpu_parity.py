@@ -101,11 +101,12 @@ def test_binning_uniform_ragged_sizes(oracle_mod, gpu, n):
     _check_mesh(oracle_mod, gpu, pos, box, ncell)
 
 
-@pytest.mark.parametrize("ncell,n", [((160, 160, 160), 300000),     # 4,096,000 cells: 22 bits -> 2 digits of 11
-                                     ((200, 170, 190), 200000),     # 6,460,000 cells: 23 bits -> 3 digits of 8
+@pytest.mark.parametrize("ncell,n", [((100, 100, 100), 300000),     # 1,000,000 cells: 20 bits -> 2 digits of 10
+                                     ((160, 160, 160), 300000),     # 4,096,000 cells: 22 bits -> 3 digits of 8
+                                     ((256, 256, 256), 200000),     # 2^24 cells (the maximum): 3 digits of 8
                                      ((3, 3, 3), 5000)])            # 27 cells: one digit of 5 bits
 def test_binning_digit_plans(oracle_mod, gpu, ncell, n):
-    """Every digit plan of the LSD counting sort (1, 2 and 3 passes; 32 ... 2048 bins), clustered input."""
+    """Every digit plan of the LSD counting sort (1, 2 and 3 passes; 32 ... 1024 bins), clustered input."""
     pos, box = workloads.scaled_clustered(n, ncell, seed=5, frac_halo=0.7, n_halo=30, a_range=(0.2, 2.0))
     _check_mesh(oracle_mod, gpu, pos, box, ncell)
 
