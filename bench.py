@@ -45,6 +45,25 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def _profiled_traffic():
+    """DRAM bytes per launch of the force kernel from the committed `ncu --set full` summary under profiles/
+    (dram__bytes_read.sum + dram__bytes_write.sum; text file, never executed).  None if the summary is absent."""
+    path = os.path.join(ROOT, "profiles", "r01_force_config4_ncu_full.txt")
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    total, seen = 0.0, 0
+    try:
+        with open(path) as fh:
+            for line in fh:
+                for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                    if line.startswith(key + " ["):
+                        u = line.split("[")[1].split("]")[0]
+                        total += float(line.split("=")[1]) * unit[u]
+                        seen += 1
+    except OSError:
+        return None
+    return total if seen == 2 else None
+
+
 # --------------------------------------------------------------------------------------- clocks --
 class ClockSampler:
     """Samples SM clock + throttle reasons of one GPU every 200 ms through NVML while the timed region runs."""
@@ -302,7 +321,10 @@ def run_product(args, w):
                    "l2": "inputs larger than L2 (16 B x N = %d MiB per array)" % (16 * n >> 20)},
         "clocks": clk, "e2e": e2e, "gpu_launches": launches,
         "roofline": {"bound": "alu", "kernel": "k_pp_force", "achieved": achieved, "peak": peak_tflops,
-                     "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None, "traffic": None,
+                     "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None,
+                     "traffic": _profiled_traffic() if args.config == 4 else None,
+                     "traffic_kind": "DRAM bytes per launch, ncu --set full capture in profiles/ (the kernel is ALU-bound: "
+                                     "algorithmic bytes are 2 x 16 B x N + cell tables, re-reads are served by L2)",
                      "peak_kind": "nominal: %d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (sm_max_mhz, %s); "
                                   "30 flop per candidate pair" % (sms, f_max_hz / 1e6, peak_kind),
                      "launch_ms": force_avg_ms, "fp32_probe": probe,

@@ -179,9 +179,7 @@ __device__ __forceinline__ void red_add_f64(double* addr, double v) {
 }
 
 struct __align__(16) WarpScratch {
-  float4 xy[kSrcTile];      // (x, x, y, y) of a staged source, relative to the item's reference point
-  float2 zz[kSrcTile];      // (z, z)
-  float2 mm[kSrcTile];      // (m, m)
+  float4 src[kSrcTile];     // (x, y, z, m) of a staged source, relative to the item's reference point
   uint32_t seg_start[kMaxSeg + 1];   // stream offset of each segment; [kMaxSeg] = S
   uint32_t seg_base[kMaxSeg];        // sorted index of each segment's first particle
   float seg_ref[kMaxSeg][3];         // integer-valued reference point R_s of the segment's cells
@@ -192,7 +190,7 @@ struct __align__(16) WarpScratch {
 template <int TP, bool kUniformMass>
 __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __restrict__ sorted, const ForceConst& fc,
                                              uint32_t tgt_begin, uint32_t tgt_end, const float ref_t[3],
-                                             uint32_t p0, uint32_t p1, double* __restrict__ acc64, int lane) {
+                                             uint32_t p0, uint32_t p1, double* __restrict__ acc64, int lane, float lane_zero) {
   // ---- targets: lane holds pairs (k, k+32) of each 64-block, negated and relative to R_t
   float2 ntx[TP], nty[TP], ntz[TP], ax[TP], ay[TP], az[TP];
 #pragma unroll
@@ -207,7 +205,11 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
     ax[t] = ay[t] = az[t] = make_float2(0.f, 0.f);
   }
   const float2 e2 = make_float2(fc.eps2, fc.eps2);
-  const float2 c5 = make_float2(fc.nq[5], fc.nq[5]), c4 = make_float2(fc.nq[4], fc.nq[4]);
+  // c5*u + c4 needs two constants in one instruction, and an FFMA2 takes at most one uniform-register operand:
+  // c4 is made a per-lane value on purpose (lane_zero is 0.0f, but not provably so), which keeps ptxas from also
+  // demoting other constants to vector registers (a third vector operand costs the FMA pipe a third cycle).
+  const float c4v = fc.nq[4] + lane_zero;
+  const float2 c5 = make_float2(fc.nq[5], fc.nq[5]), c4 = make_float2(c4v, c4v);
   const float2 c3 = make_float2(fc.nq[3], fc.nq[3]), c2 = make_float2(fc.nq[2], fc.nq[2]);
   const float2 c1 = make_float2(fc.nq[1], fc.nq[1]), c0 = make_float2(fc.nq[0], fc.nq[0]);
   const float rc2e = fc.rc2e;
@@ -219,32 +221,26 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
 #pragma unroll
     for (int j = 0; j < kSrcTile / 32; ++j) {
       const uint32_t p = tile + j * 32 + lane;
-      float4 xy = make_float4(1.0e3f, 1.0e3f, 1.0e3f, 1.0e3f);
-      float2 zz = make_float2(1.0e3f, 1.0e3f), mm = make_float2(0.f, 0.f);
+      float4 sv = make_float4(1.0e3f, 1.0e3f, 1.0e3f, 0.f);
       if (p < p1) {
         while (p >= ws.seg_start[seg + 1]) ++seg;
         const float4 v = __ldg(&sorted[ws.seg_base[seg] + (p - ws.seg_start[seg])]);
         const float x = (v.x - ws.seg_ref[seg][0]) + ws.seg_delta[seg][0];
         const float y = (v.y - ws.seg_ref[seg][1]) + ws.seg_delta[seg][1];
         const float z = (v.z - ws.seg_ref[seg][2]) + ws.seg_delta[seg][2];
-        xy = make_float4(x, x, y, y);
-        zz = make_float2(z, z);
-        mm = make_float2(v.w, v.w);
+        sv = make_float4(x, y, z, v.w);
       }
-      ws.xy[j * 32 + lane] = xy;
-      ws.zz[j * 32 + lane] = zz;
-      if (!kUniformMass) ws.mm[j * 32 + lane] = mm;
+      ws.src[j * 32 + lane] = sv;
     }
     __syncwarp();
     // ---- pair loop: every source of the tile against the lane's 2*TP targets
     const int cnt = (int)min((uint32_t)kSrcTile, (p1 - tile + 3u) & ~3u);
 #pragma unroll 4
     for (int j = 0; j < cnt; ++j) {
-      const float4 sxy = ws.xy[j];
-      const float2 sz = ws.zz[j];
-      const float2 sx = make_float2(sxy.x, sxy.y), sy = make_float2(sxy.z, sxy.w);
-      float2 sm;
-      if (!kUniformMass) sm = ws.mm[j];
+      // one LDS.128 per source; the packed instructions broadcast the scalar to both halves (R.F32 operand form)
+      const float4 sv = ws.src[j];
+      const float2 sx = make_float2(sv.x, sv.x), sy = make_float2(sv.y, sv.y), sz = make_float2(sv.z, sv.z);
+      const float2 sm = make_float2(sv.w, sv.w);
 #pragma unroll
       for (int t = 0; t < TP; ++t) {
         const float2 dx = __fadd2_rn(sx, ntx[t]);
@@ -296,6 +292,7 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
   const int lane = threadIdx.x & 31;
   WarpScratch& ws = scratch[threadIdx.x >> 5];
   const unsigned long long total = flags->total_items;
+  const float lane_zero = __uint_as_float(__ldg(&flags->pad0 + (lane >> 5)));   // 0.0f (pad0 is cleared by every mesh build)
 
   for (;;) {
     unsigned long long idx = 0;
@@ -356,9 +353,9 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
     const uint32_t p0 = chunk * kSrcChunk, p1 = min(S, p0 + kSrcChunk);
     const uint32_t tb = cs0 + tile * 32u * T, te = min(cs1, tb + 32u * T);
     if (T == 2)
-      process_item<1, kUniformMass>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane);
+      process_item<1, kUniformMass>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
     else
-      process_item<2, kUniformMass>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane);
+      process_item<2, kUniformMass>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
   }
 }
 
