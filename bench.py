@@ -306,7 +306,9 @@ def run_product(args, w):
     peak_tflops = sms * FP32_LANES_PER_SM * 2 * f_max_hz / 1e12
     force_avg_ms = float(np.mean(force_ms)) if force_ms else None
     achieved = FLOP_PER_PAIR * W / (force_avg_ms * 1e-3) / 1e12 if force_avg_ms else None
-    probe = {"ffma_tflops": sol.probe_fp32(0, 4000) / 1e12, "ffma2_tflops": sol.probe_fp32(1, 4000) / 1e12}
+    probe = {"ffma_tflops": sol.probe_fp32(0, 4000) / 1e12, "ffma2_tflops": sol.probe_fp32(1, 4000) / 1e12,
+             "ffma2_2_vector_operands_tflops": sol.probe_fp32(2, 4000) / 1e12,
+             "ffma2_3_vector_operands_tflops": sol.probe_fp32(3, 4000) / 1e12}
     ncells = w.ncell[0] * w.ncell[1] * w.ncell[2]
     bin_bytes = BIN_BYTES_PER_PARTICLE * n + 8 * ncells
     mesh_avg_ms = float(np.mean(mesh_ms)) if mesh_ms else None

@@ -123,8 +123,9 @@ int32_t srpp_get_timings(srpp_ctx* ctx, srpp_timings* timings_host);
 
 /* FP32 peak probe for the "% of FP32 peak" report: runs a register-only FMA stream on
  * every SM of the context's device and writes the sustained flop/s to *flops_per_s_host.
- * variant 0 = scalar FFMA, 1 = packed FFMA2 (the pair loop's form); trips >= 1 scales the run time
- * (trips = 2000 is about 10 ms).  Synchronises. */
+ * variant 0 = scalar FFMA, 1 = packed FFMA2 (the pair loop's form), 2 / 3 = packed FFMA2 whose every
+ * instruction reads 2 / 3 different vector registers (register-file operand bandwidth);
+ * trips >= 1 scales the run time (trips = 2000 is about 10 ms).  Synchronises. */
 int32_t srpp_probe_fp32(srpp_ctx* ctx, int32_t variant, int32_t trips, double* flops_per_s_host);
 
 /* A7: sub-cycled kick, v <- fmaf(a, kdt, v) per component in fp32 (R16); .w lanes untouched.

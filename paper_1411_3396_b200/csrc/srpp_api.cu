@@ -208,7 +208,7 @@ int32_t srpp_get_timings(srpp_ctx* c, srpp_timings* t) {
 }
 
 int32_t srpp_probe_fp32(srpp_ctx* c, int32_t variant, int32_t trips, double* flops_per_s_host) {
-  if (!c || !flops_per_s_host || variant < 0 || variant > 1 || trips < 1) return SRPP_ERR_INVALID_ARG;
+  if (!c || !flops_per_s_host || variant < 0 || variant > 3 || trips < 1) return SRPP_ERR_INVALID_ARG;
   // scratch word: the unused tail of the 256-byte flag block at the head of the workspace
   static_assert(sizeof(DevFlags) <= 128, "flag block layout");
   const cudaError_t e = run_fp32_probe(c->stream, variant, trips, flops_per_s_host, (float*)(c->ws + 128));
