@@ -362,10 +362,25 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
 // --------------------------------------------------------------------------------- A6: write-back --
 __global__ void __launch_bounds__(256) k_write_back(const double* __restrict__ acc64, const uint32_t* __restrict__ perm,
                                                      int64_t n, float scale, float4* __restrict__ acc) {
-  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
-    const double s = (double)scale;
-    const float ax = (float)(acc64[3 * k + 0] * s), ay = (float)(acc64[3 * k + 1] * s), az = (float)(acc64[3 * k + 2] * s);
-    acc[__ldg(&perm[k])] = make_float4(ax, ay, az, 0.f);
+  // 4 independent elements per thread and trip: the scattered 16-byte stores are the slow part, keep many in flight
+  constexpr int U = 4;
+  const double s = (double)scale;
+  for (int64_t k0 = (int64_t)blockIdx.x * blockDim.x * U + threadIdx.x; k0 < n; k0 += (int64_t)gridDim.x * blockDim.x * U) {
+    double a[U][3];
+    uint32_t dst[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t k = k0 + (int64_t)u * blockDim.x;
+      if (k < n) {
+        dst[u] = __ldcs(&perm[k]);
+        a[u][0] = __ldcs(&acc64[3 * k + 0]); a[u][1] = __ldcs(&acc64[3 * k + 1]); a[u][2] = __ldcs(&acc64[3 * k + 2]);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t k = k0 + (int64_t)u * blockDim.x;
+      if (k < n) acc[dst[u]] = make_float4((float)(a[u][0] * s), (float)(a[u][1] * s), (float)(a[u][2] * s), 0.f);
+    }
   }
 }
 
@@ -432,7 +447,8 @@ cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
     k_pp_force<false><<<grid, kForceThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
   if (c->timing) cudaEventRecord(c->ev[kEvForce1], st);
   const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
-  k_write_back<<<grid_ew, 256, 0, st>>>(c->acc64, c->perm, n, c->uniform_mass ? c->mass0 : 1.0f, acc);
+  const int grid_wb = (int)std::min<int64_t>((n + 1023) / 1024, (int64_t)c->num_sms * 16);
+  k_write_back<<<grid_wb, 256, 0, st>>>(c->acc64, c->perm, n, c->uniform_mass ? c->mass0 : 1.0f, acc);
   c->launches += 6;
   if (c->timing) { cudaEventRecord(c->ev[kEvAccel1], st); c->ev_accel_valid = true; }
   return cudaGetLastError();
