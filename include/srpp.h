@@ -128,6 +128,20 @@ int32_t srpp_get_timings(srpp_ctx* ctx, srpp_timings* timings_host);
  * trips >= 1 scales the run time (trips = 2000 is about 10 ms).  Synchronises. */
 int32_t srpp_probe_fp32(srpp_ctx* ctx, int32_t variant, int32_t trips, double* flops_per_s_host);
 
+/* Overloaded (non-periodic) node volume and active/passive particles ("particle
+ * overloading", PAPER.md:73 blocks of active and passive particles).  Optional; the default after srpp_create is a fully
+ * periodic box in which every particle is active (BASELINE.json configs).
+ *   periodic_host[3]   1 = periodic axis (minimum image), 0 = open axis: coordinate differences are taken as they are
+ *                      and the 27-cell stencil stops at the box faces.  NULL = all periodic.
+ *   active_lo_host[3], active_hi_host[3]   the active box.  Accelerations are computed for every particle in a
+ *                      chaining-mesh cell that intersects [lo, hi) (a superset of the particles inside it); particles in
+ *                      the other cells are passive: they act as sources only and their acceleration is written as 0.
+ *                      NULL = the whole box.
+ * Host pointers, read during the call.  Takes effect at the next srpp_accel (the mesh does not depend on it).
+ * Errors: INVALID_ARG (null ctx, lo > hi, non-finite). */
+int32_t srpp_set_boundary(srpp_ctx* ctx, const int32_t* periodic_host, const float* active_lo_host,
+                          const float* active_hi_host);
+
 /* A7: sub-cycled kick, v <- fmaf(a, kdt, v) per component in fp32 (R16); .w lanes untouched.
  * vel, acc: device float4[n].  Asynchronous. */
 int32_t srpp_kick(srpp_ctx* ctx, float* vel, const float* acc, float kdt, int64_t n);

@@ -39,11 +39,16 @@ DEFAULT_POLY = np.array(DEFAULT_POLY_BITS, dtype=np.uint32).view(np.float32)
 
 
 class Params(C.Structure):
-    _fields_ = [("box", C.c_float * 3), ("rcut", C.c_float), ("eps", C.c_float), ("poly", C.c_float * 6)]
+    _fields_ = [("box", C.c_float * 3), ("rcut", C.c_float), ("eps", C.c_float), ("poly", C.c_float * 6),
+                ("periodic", C.c_int32 * 3)]
 
 
-def make_params(box, rcut=3.0, eps=0.1, poly=None) -> Params:
+def make_params(box, rcut=3.0, eps=0.1, poly=None, periodic=(1, 1, 1)) -> Params:
+    """periodic[a] = 0 makes axis a open: plain coordinate differences, no neighbours across the faces (the
+    overloaded node volume of PAPER.md:65); the default is the periodic box of BASELINE.json."""
     p = Params()
+    for a in range(3):
+        p.periodic[a] = 1 if periodic[a] else 0
     for a in range(3):
         p.box[a] = float(box[a])
     p.rcut = float(rcut)

@@ -53,6 +53,8 @@ typedef struct {
   float rcut;
   float eps;
   float poly[6];
+  int32_t periodic[3]; /* 1: periodic axis, minimum image (R8); 0: open axis, plain differences and no neighbours
+                          across the faces -- the overloaded (non-periodic) node volume of PAPER.md:65 */
 } orc_params;
 
 int32_t orc_num_threads(void) {
@@ -147,6 +149,9 @@ static inline double min_image(double d, double L) {
   return d;
 }
 
+/* coordinate difference on one axis: minimum image if the axis is periodic, the plain difference if it is open */
+static inline double axis_diff(double d, double L, int32_t periodic) { return periodic ? min_image(d, L) : d; }
+
 /*
  * The plain definition, O(N^2): for every target i the sum over ALL j != i.
  * acc[3n] fp64.  Optional outputs (may be NULL): n_in[n] = number of in-cutoff neighbours,
@@ -166,9 +171,9 @@ void orc_accel_bruteforce(const float *pos_mass, int64_t n, const orc_params *p,
     int64_t cnt = 0;
     for (int64_t j = 0; j < n; ++j) {
       if (j == i) continue; /* R7 */
-      double dx = min_image((double)pos_mass[4 * j] - xi, L[0]);
-      double dy = min_image((double)pos_mass[4 * j + 1] - yi, L[1]);
-      double dz = min_image((double)pos_mass[4 * j + 2] - zi, L[2]);
+      double dx = axis_diff((double)pos_mass[4 * j] - xi, L[0], p->periodic[0]);
+      double dy = axis_diff((double)pos_mass[4 * j + 1] - yi, L[1], p->periodic[1]);
+      double dz = axis_diff((double)pos_mass[4 * j + 2] - zi, L[2], p->periodic[2]);
       double s = dx * dx + dy * dy + dz * dz;
       if (s < rc2) { /* strict cutoff on the unsoftened s (R5) */
         double u = s + e2;
@@ -264,17 +269,22 @@ int32_t orc_accel(const float *pos_mass, int64_t n, const orc_params *p, const i
     for (int oz = lo[2]; oz <= hi[2]; ++oz)
       for (int oy = lo[1]; oy <= hi[1]; ++oy)
         for (int ox = lo[0]; ox <= hi[0]; ++ox) {
-          int32_t cx = (ci[0] + ox + g.nc[0]) % g.nc[0];
-          int32_t cy = (ci[1] + oy + g.nc[1]) % g.nc[1];
-          int32_t cz = (ci[2] + oz + g.nc[2]) % g.nc[2];
+          int32_t cx = ci[0] + ox, cy = ci[1] + oy, cz = ci[2] + oz;
+          /* open axis: no neighbour cell beyond the faces; periodic axis: wrap */
+          if ((!p->periodic[0] && (cx < 0 || cx >= g.nc[0])) || (!p->periodic[1] && (cy < 0 || cy >= g.nc[1])) ||
+              (!p->periodic[2] && (cz < 0 || cz >= g.nc[2])))
+            continue;
+          cx = (cx + g.nc[0]) % g.nc[0];
+          cy = (cy + g.nc[1]) % g.nc[1];
+          cz = (cz + g.nc[2]) % g.nc[2];
           int64_t cc = cx + g.nc[0] * (cy + (int64_t)g.nc[1] * cz);
           for (uint32_t q = g.start[cc]; q < g.start[cc + 1]; ++q) {
             int64_t j = g.order[q];
             if (j == i) continue; /* R7 */
             ++cand;
-            double dx = min_image((double)pos_mass[4 * j] - xi, L[0]);
-            double dy = min_image((double)pos_mass[4 * j + 1] - yi, L[1]);
-            double dz = min_image((double)pos_mass[4 * j + 2] - zi, L[2]);
+            double dx = axis_diff((double)pos_mass[4 * j] - xi, L[0], p->periodic[0]);
+            double dy = axis_diff((double)pos_mass[4 * j + 1] - yi, L[1], p->periodic[1]);
+            double dz = axis_diff((double)pos_mass[4 * j + 2] - zi, L[2], p->periodic[2]);
             double s = dx * dx + dy * dy + dz * dz;
             double m = (double)pos_mass[4 * j + 3];
             if (s < rc2) {

@@ -20,7 +20,7 @@ STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "GEOMETRY", -3: "DOMAIN", -4: "W
 EXPORTS = ("srpp_version", "srpp_default_poly", "srpp_workspace_bytes", "srpp_create", "srpp_destroy",
            "srpp_build_mesh", "srpp_get_mesh", "srpp_accel", "srpp_get_stats", "srpp_kick", "srpp_stream",
            "srpp_step_host", "srpp_strerror", "srpp_last_cuda_error", "srpp_set_timing", "srpp_get_timings",
-           "srpp_probe_fp32")
+           "srpp_probe_fp32", "srpp_set_boundary")
 
 
 class SrppParams(C.Structure):
@@ -84,6 +84,8 @@ def load() -> C.CDLL:
     L.srpp_set_timing.argtypes = [vp, i32]
     L.srpp_get_timings.restype = i32
     L.srpp_get_timings.argtypes = [vp, C.POINTER(SrppTimings)]
+    L.srpp_set_boundary.restype = i32
+    L.srpp_set_boundary.argtypes = [vp, C.POINTER(i32), C.POINTER(C.c_float), C.POINTER(C.c_float)]
     L.srpp_probe_fp32.restype = i32
     L.srpp_probe_fp32.argtypes = [vp, i32, i32, C.POINTER(C.c_double)]
     L.srpp_strerror.restype = C.c_char_p
@@ -231,6 +233,13 @@ class Solver:
         t = SrppTimings()
         self._check(self.lib.srpp_get_timings(self._ctx, C.byref(t)), "srpp_get_timings")
         return {k: float(getattr(t, k)) for k, _ in SrppTimings._fields_}
+
+    def set_boundary(self, periodic=(1, 1, 1), active_lo=None, active_hi=None) -> None:
+        """srpp_set_boundary: open (non-periodic) axes and the active box of an overloaded node volume."""
+        per = (C.c_int32 * 3)(*[1 if v else 0 for v in periodic])
+        lo = (C.c_float * 3)(*[float(v) for v in active_lo]) if active_lo is not None else None
+        hi = (C.c_float * 3)(*[float(v) for v in active_hi]) if active_hi is not None else None
+        self._check(self.lib.srpp_set_boundary(self._ctx, per, lo, hi), "srpp_set_boundary")
 
     def probe_fp32(self, variant: int = 1, trips: int = 2000) -> float:
         """Sustained FP32 flop/s of a register-only FMA stream (0 = FFMA, 1 = packed FFMA2)."""

@@ -126,6 +126,9 @@ int32_t srpp_create(srpp_ctx** out, const srpp_params* params, void* workspace, 
     g.inv_cell[a] = (float)params->ncell[a] / params->box[a];   // one IEEE fp32 division (R10)
     g.cell_w[a] = params->box[a] / (float)params->ncell[a];
     ncells *= params->ncell[a];
+    g.periodic[a] = 1;
+    g.act_lo[a] = 0;
+    g.act_hi[a] = params->ncell[a];
   }
   g.ncells = (int32_t)ncells;
   plan_sort(g.ncells, &c->sort_passes, &c->sort_digit_bits);
@@ -214,6 +217,31 @@ int32_t srpp_probe_fp32(srpp_ctx* c, int32_t variant, int32_t trips, double* flo
   const cudaError_t e = run_fp32_probe(c->stream, variant, trips, flops_per_s_host, (float*)(c->ws + 128));
   if (e != cudaSuccess) return cuda_fail(c, e);
   c->launches += 2;
+  return SRPP_OK;
+}
+
+int32_t srpp_set_boundary(srpp_ctx* c, const int32_t* periodic_host, const float* active_lo_host,
+                          const float* active_hi_host) {
+  if (!c) return SRPP_ERR_INVALID_ARG;
+  Geometry& g = c->geo;
+  for (int a = 0; a < 3; ++a) {
+    const int32_t per = periodic_host ? (periodic_host[a] != 0) : 1;
+    float lo = active_lo_host ? active_lo_host[a] : 0.f, hi = active_hi_host ? active_hi_host[a] : c->params.box[a];
+    if (!(lo <= hi) || !isfinite(lo) || !isfinite(hi)) return SRPP_ERR_INVALID_ARG;
+    lo = fmaxf(lo, 0.f);
+    hi = fminf(hi, c->params.box[a]);
+    // cells [clo, chi) that can hold a particle with lo <= x < hi: the fp32 cell function of A1 (R10) is monotonic
+    // in x, so the cells of lo and of the largest float below hi bound the range
+    int32_t clo = (int32_t)floorf(lo * g.inv_cell[a]);
+    int32_t chi = (int32_t)floorf(nextafterf(hi, -INFINITY) * g.inv_cell[a]) + 1;
+    if (clo > g.ncell[a] - 1) clo = g.ncell[a] - 1;
+    if (clo < 0) clo = 0;
+    if (chi > g.ncell[a]) chi = g.ncell[a];
+    if (hi <= lo) chi = clo;
+    g.periodic[a] = per;
+    g.act_lo[a] = clo;
+    g.act_hi[a] = chi;
+  }
   return SRPP_OK;
 }
 

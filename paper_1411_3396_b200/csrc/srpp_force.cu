@@ -40,17 +40,21 @@ __device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint
   const int dy = row % 3 - 1, dz = row / 3 - 1;
   int y = cy + dy, z = cz + dz;
   s.shift[0] = 0.f; s.shift[1] = 0.f; s.shift[2] = 0.f;
-  if (y < 0) { y += g.ncell[1]; s.shift[1] = -g.box[1]; } else if (y >= g.ncell[1]) { y -= g.ncell[1]; s.shift[1] = g.box[1]; }
-  if (z < 0) { z += g.ncell[2]; s.shift[2] = -g.box[2]; } else if (z >= g.ncell[2]) { z -= g.ncell[2]; s.shift[2] = g.box[2]; }
+  bool empty = false;
+  if (y < 0) { y += g.ncell[1]; s.shift[1] = -g.box[1]; empty |= !g.periodic[1]; }
+  else if (y >= g.ncell[1]) { y -= g.ncell[1]; s.shift[1] = g.box[1]; empty |= !g.periodic[1]; }
+  if (z < 0) { z += g.ncell[2]; s.shift[2] = -g.box[2]; empty |= !g.periodic[2]; }
+  else if (z >= g.ncell[2]) { z -= g.ncell[2]; s.shift[2] = g.box[2]; empty |= !g.periodic[2]; }
   const int ncx = g.ncell[0];
   int xlo, xhi;  // inclusive; xhi < xlo means empty
   if (cx >= 1 && cx <= ncx - 2) {
     if (sx == 0) { xlo = cx - 1; xhi = cx + 1; } else { xlo = 0; xhi = -1; }
   } else if (cx == 0) {
-    if (sx == 0) { xlo = ncx - 1; xhi = ncx - 1; s.shift[0] = -g.box[0]; } else { xlo = 0; xhi = 1; }
+    if (sx == 0) { xlo = ncx - 1; xhi = g.periodic[0] ? ncx - 1 : ncx - 2; s.shift[0] = -g.box[0]; } else { xlo = 0; xhi = 1; }
   } else {
-    if (sx == 0) { xlo = ncx - 2; xhi = ncx - 1; } else { xlo = 0; xhi = 0; s.shift[0] = g.box[0]; }
+    if (sx == 0) { xlo = ncx - 2; xhi = ncx - 1; } else { xlo = 0; xhi = g.periodic[0] ? 0 : -1; s.shift[0] = g.box[0]; }
   }
+  if (empty) xhi = xlo - 1;   // the (dy,dz) row lies beyond an open face
   s.xlo = xlo; s.cy = y; s.cz = z;
   if (xhi < xlo) { s.start = 0; s.end = 0; return s; }
   const int rowbase = ncx * (y + g.ncell[1] * z);
@@ -70,8 +74,10 @@ __global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__
   if (c < g.ncells) {
     const uint32_t n_c = __ldg(&cell_start[c + 1]) - __ldg(&cell_start[c]);
     unsigned long long it = 0;
-    if (n_c) {
-      const int cx = c % g.ncell[0], cy = (c / g.ncell[0]) % g.ncell[1], cz = c / (g.ncell[0] * g.ncell[1]);
+    const int cx = c % g.ncell[0], cy = (c / g.ncell[0]) % g.ncell[1], cz = c / (g.ncell[0] * g.ncell[1]);
+    const bool active = cx >= g.act_lo[0] && cx < g.act_hi[0] && cy >= g.act_lo[1] && cy < g.act_hi[1] &&
+                        cz >= g.act_lo[2] && cz < g.act_hi[2];
+    if (n_c && active) {
       unsigned long long S = 0;
       for (int seg = 0; seg < kMaxSeg; ++seg) {
         const Segment s = stencil_segment(g, cell_start, cx, cy, cz, seg);

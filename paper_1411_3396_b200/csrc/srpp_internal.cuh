@@ -47,6 +47,9 @@ struct Geometry {
   float cell_w[3];       // box / ncell (fp32), only used to pick integer reference points
   int32_t ncell[3];
   int32_t ncells;
+  int32_t periodic[3];   // 1: periodic axis (stencil wraps, image shift); 0: open axis (stencil stops at the faces)
+  int32_t act_lo[3];     // cells [act_lo, act_hi) per axis hold the ACTIVE targets; the other cells are passive
+  int32_t act_hi[3];     //   (sources only) -- the overloaded node volume of PAPER.md:65/73
 };
 
 struct ForceConst {

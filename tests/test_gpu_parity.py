@@ -370,3 +370,72 @@ def test_config4_full_size_sampled(oracle_mod, gpu):
 @pytest.mark.parametrize("cfg", [3, 5])
 def test_configs_3_5_full_size_sampled(oracle_mod, gpu, cfg):
     _full_config(oracle_mod, gpu, cfg, 512, 512)
+
+
+# ---------------------------------------- open axes and active/passive particles (overloaded node volume) --
+
+def _gpu_accel_boundary(gpu, pos, box, ncell, eps, periodic, lo=None, hi=None):
+    torch, binding = gpu
+    sol = _solver(gpu, box, ncell, eps, pos.shape[0])
+    sol.set_boundary(periodic, lo, hi)
+    d = torch.from_numpy(np.ascontiguousarray(pos)).cuda()
+    sol.build_mesh(d)
+    acc = sol.accel()
+    torch.cuda.synchronize()
+    return acc.cpu().numpy(), sol
+
+
+@pytest.mark.parametrize("periodic", [(0, 0, 0), (1, 0, 1), (0, 1, 0)])
+def test_accel_open_axes(oracle_mod, gpu, periodic):
+    """srpp_set_boundary with open axes against the oracle's plain-difference sum."""
+    ncell = (6, 5, 7)
+    pos, box = workloads.scaled_clustered(50000, ncell, seed=31, frac_halo=0.6, n_halo=10, a_range=(0.2, 1.5))
+    a, sol = _gpu_accel_boundary(gpu, pos, box, ncell, 0.05, periodic)
+    prm = oracle_mod.make_params(box, 3.0, 0.05, periodic=periodic)
+    ref, st = oracle_mod.accel(pos, prm, stats=True)
+    per, glob = oracle_mod.error_norms(a, ref, st["allowance"])
+    assert per.max() <= PER_PARTICLE_TOL and glob <= GLOBAL_L2_TOL, (per.max(), glob)
+    # the open box has fewer candidate pairs than the periodic one
+    a2, sol2 = _gpu_accel_boundary(gpu, pos, box, ncell, 0.05, (1, 1, 1))
+    assert sol.get_stats()["candidate_pairs"] < sol2.get_stats()["candidate_pairs"]
+
+
+def test_accel_active_box(oracle_mod, gpu):
+    """Only cells that intersect the active box get work; passive particles are sources and come back as 0."""
+    ncell = (8, 6, 7)
+    pos, box = workloads.scaled_clustered(60000, ncell, seed=32, frac_halo=0.5, n_halo=12, a_range=(0.2, 1.5))
+    lo, hi = (3.2 * 2, 3.2 * 1, 0.0), (3.2 * 6, 3.2 * 5, box[2])
+    a, sol = _gpu_accel_boundary(gpu, pos, box, ncell, 0.05, (0, 0, 1), lo, hi)
+    inside = np.all((pos[:, :3] >= np.asarray(lo, dtype=np.float32)) & (pos[:, :3] < np.asarray(hi, dtype=np.float32)), axis=1)
+    prm = oracle_mod.make_params(box, 3.0, 0.05, periodic=(0, 0, 1))
+    t = np.nonzero(inside)[0]
+    ref, st = oracle_mod.accel(pos, prm, targets=t, stats=True)
+    per, glob = oracle_mod.error_norms(a[t], ref, st["allowance"])
+    assert per.max() <= PER_PARTICLE_TOL and glob <= GLOBAL_L2_TOL, (per.max(), glob)
+    # cells entirely outside the active box: exact zeros
+    cid = oracle_mod.cell_ids(pos, box, ncell)
+    cx, cy = cid % ncell[0], (cid // ncell[0]) % ncell[1]
+    passive = (cx < 2) | (cx >= 6) | (cy < 1) | (cy >= 5)
+    assert passive.any() and np.all(a[passive] == 0.0)
+
+
+def test_overloaded_subvolume_reproduces_periodic_box(oracle_mod, gpu):
+    """The point of overloading: a node that holds its own slab plus a shell of passive copies at
+    least rc wide, with OPEN faces, gets the same accelerations for its active particles as the full periodic box."""
+    ncell = (10, 5, 6)
+    pos, box = workloads.scaled_clustered(80000, ncell, seed=33, frac_halo=0.5, n_halo=15, a_range=(0.2, 1.5))
+    cell = np.float32(3.2)
+    x0, x1 = 3 * cell, 7 * cell                       # active slab: cells 3..6 along x
+    keep = (pos[:, 0] >= x0 - cell) & (pos[:, 0] < x1 + cell)
+    sub = pos[keep].copy()
+    sub[:, 0] -= (x0 - cell)                          # exact: multiples of 3.2 in [0, 32) are fp32-exact differences?
+    sub_box = (float(6 * cell), box[1], box[2])
+    sub[:, 0] = np.clip(sub[:, 0], 0, np.nextafter(np.float32(sub_box[0]), np.float32(0)))
+    a, sol = _gpu_accel_boundary(gpu, sub, sub_box, (6, ncell[1], ncell[2]), 0.05, (0, 1, 1),
+                                 (float(cell), 0.0, 0.0), (float(5 * cell), box[1], box[2]))
+    active_full = np.nonzero(keep)[0][(pos[keep, 0] >= x0) & (pos[keep, 0] < x1)]
+    active_sub = np.nonzero((pos[keep, 0] >= x0) & (pos[keep, 0] < x1))[0]
+    ref, st = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, 0.05), targets=active_full, stats=True)
+    # the shifted coordinates differ from the originals by an fp32 rounding, so allow twice the usual global bar
+    per, glob = oracle_mod.error_norms(a[active_sub], ref, st["allowance"])
+    assert per.max() <= PER_PARTICLE_TOL and glob <= 2 * GLOBAL_L2_TOL, (per.max(), glob)

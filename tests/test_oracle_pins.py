@@ -340,3 +340,51 @@ def test_kick_and_stream(oracle_mod):
     d -= np.asarray(box) * np.round(d / np.asarray(box))
     assert np.max(np.abs(d)) < 4e-6
     oracle_mod.cell_ids(x1, box, (5, 5, 10))   # stays in the domain
+
+
+# ------------------------------------------------- open (non-periodic) axes: the overloaded node volume --
+# PAPER.md:65 ("particle overloading"): a node evolves its own volume plus a shell of passive copies, with no wrap.
+# The oracle's `periodic` flags select plain coordinate differences per axis.
+
+@pytest.mark.parametrize("periodic", [(0, 0, 0), (1, 0, 1), (0, 1, 1)])
+@pytest.mark.parametrize("seed", [1, 2])
+def test_open_axes_bruteforce_vs_cell_list(oracle_mod, periodic, seed):
+    """The O(N^2) definition with plain differences on the open axes against the oracle's own cell list."""
+    ncell = (4, 3, 5)
+    pos, box = workloads.scaled_clustered(1500, ncell, seed=seed, frac_halo=0.6, n_halo=4, a_range=(0.3, 1.5))
+    prm = oracle_mod.make_params(box, 3.0, 0.07, periodic=periodic)
+    brute = oracle_mod.accel_bruteforce(pos, prm)
+    cell = oracle_mod.accel(pos, prm)
+    scale = np.abs(brute).max()
+    assert np.abs(cell - brute).max() <= 1e-12 * scale
+    # and the open result really differs from the periodic one (particles near the faces lose their images)
+    per = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, 0.07))
+    assert np.abs(per - cell).max() > 1e-6 * scale
+
+
+def test_open_axis_pair_across_the_face(oracle_mod):
+    """Closed form: two particles 0.75 apart through the x wrap attract in the periodic box and do not see each
+    other when x is open; along y (still periodic) nothing changes."""
+    box = (16.0, 16.0, 16.0)
+    pos = np.array([[0.5, 8.0, 8.0, 1.0], [15.75, 8.0, 8.0, 1.0]], dtype=np.float32)
+    eps = 0.1
+    a_per = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, eps))
+    prm = oracle_mod.make_params(box, 3.0, eps)
+    f = oracle_mod.pair_factor(prm, 0.75 ** 2)
+    assert a_per[0, 0] == pytest.approx(-0.75 * f, rel=1e-14) and a_per[1, 0] == pytest.approx(0.75 * f, rel=1e-14)
+    a_open = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, eps, periodic=(0, 1, 1)))
+    assert np.all(a_open == 0.0)
+    a_open_y = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, eps, periodic=(1, 0, 1)))
+    assert np.array_equal(a_open_y, a_per)
+
+
+def test_open_equals_periodic_when_no_pair_wraps(oracle_mod):
+    """If every particle lies in a sub-box of extent <= L - rc per axis, no minimum image is shorter than rc other
+    than the plain difference: open and periodic sums are the same arithmetic."""
+    rng = np.random.default_rng(5)
+    box = (20.0, 18.0, 22.0)
+    pos = np.ones((3000, 4), dtype=np.float32)
+    pos[:, :3] = (1.0 + rng.random((3000, 3)) * (np.asarray(box) - 3.0 - 1.0)).astype(np.float32)
+    a_per = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, 0.1))
+    a_open = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, 0.1, periodic=(0, 0, 0)))
+    assert np.array_equal(a_per, a_open)
