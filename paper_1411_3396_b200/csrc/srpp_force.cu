@@ -63,7 +63,13 @@ __device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint
   return s;
 }
 
-__device__ __forceinline__ int targets_per_lane(uint32_t n_c) { return n_c <= 64u ? 2 : 4; }
+// Targets of one work item.  Large cells: 32 lanes x 4 targets (two packed pairs per lane).  Cells of <= 64
+// particles (the uniform background: ~33 per cell) would leave half of a 64-target tile empty, so there the warp is
+// split 4 ways over the SOURCES: 8 lanes x 2 targets = 16 targets per item, lane group g = lane / 8 takes sources
+// g, g+4, g+8, ... of the staged tile, and the four partial sums are added with shuffles at the end.
+constexpr int kSmallCell = 64;
+constexpr int kSplit = 4;                       // source phases of the small-cell path
+__device__ __forceinline__ uint32_t targets_per_item(uint32_t n_c) { return n_c <= (uint32_t)kSmallCell ? 64u / kSplit : 128u; }
 
 // ------------------------------------------------------------------- plan: items per cell, W, max --
 __global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__ cell_start, Geometry g,
@@ -83,12 +89,12 @@ __global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__
         const Segment s = stencil_segment(g, cell_start, cx, cy, cz, seg);
         S += s.end - s.start;
       }
-      const int T = targets_per_lane(n_c);
-      const unsigned long long ntile = (n_c + 32u * T - 1) / (32u * T);
+      const uint32_t tpi = targets_per_item(n_c);
+      const unsigned long long ntile = (n_c + tpi - 1) / tpi;
       const unsigned long long nchunk = (S + kSrcChunk - 1) / kSrcChunk;
       it = ntile * nchunk;
       w = (unsigned long long)n_c * S;
-      slots = ntile * 32ull * T * ((S + 3ull) & ~3ull);
+      slots = ntile * tpi * ((S + 3ull) & ~3ull);
       nmax = n_c;
     }
     items[c] = it;
@@ -193,7 +199,7 @@ struct __align__(16) WarpScratch {
 };
 
 // One work item for one warp.  TP = target pairs per lane (T = 2*TP targets per lane).
-template <int TP, bool kUniformMass>
+template <int TP, bool kUniformMass, int S>
 __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __restrict__ sorted, const ForceConst& fc,
                                              uint32_t tgt_begin, uint32_t tgt_end, const float ref_t[3],
                                              uint32_t p0, uint32_t p1, double* __restrict__ acc64, int lane, float lane_zero) {
@@ -201,7 +207,7 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
   float2 ntx[TP], nty[TP], ntz[TP], ax[TP], ay[TP], az[TP];
 #pragma unroll
   for (int t = 0; t < TP; ++t) {
-    const uint32_t k0 = tgt_begin + t * 64 + lane, k1 = k0 + 32;
+    const uint32_t k0 = tgt_begin + t * (64 / S) + (lane & (32 / S - 1)), k1 = k0 + 32 / S;
     float4 a = make_float4(-1.0e3f, -1.0e3f, -1.0e3f, 0.f), b = a;
     if (k0 < tgt_end) { a = __ldg(&sorted[k0]); a.x -= ref_t[0]; a.y -= ref_t[1]; a.z -= ref_t[2]; }
     if (k1 < tgt_end) { b = __ldg(&sorted[k1]); b.x -= ref_t[0]; b.y -= ref_t[1]; b.z -= ref_t[2]; }
@@ -242,7 +248,7 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
     // ---- pair loop: every source of the tile against the lane's 2*TP targets
     const int cnt = (int)min((uint32_t)kSrcTile, (p1 - tile + 3u) & ~3u);
 #pragma unroll 4
-    for (int j = 0; j < cnt; ++j) {
+    for (int j = (S > 1 ? lane / (32 / S) : 0); j < cnt; j += S) {
       // one LDS.128 per source; the packed instructions broadcast the scalar to both halves (R.F32 operand form)
       const float4 sv = ws.src[j];
       const float2 sx = make_float2(sv.x, sv.x), sy = make_float2(sv.y, sv.y), sz = make_float2(sv.z, sv.z);
@@ -272,10 +278,23 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
       }
     }
   }
+  // ---- small-cell path: add the partial sums of the S source phases (lanes l, l + 32/S, ... hold the same targets)
+  if (S > 1) {
+#pragma unroll
+    for (int t = 0; t < TP; ++t) {
+#pragma unroll
+      for (int o = 32 / S; o < 32; o <<= 1) {
+        ax[t].x += __shfl_xor_sync(0xffffffffu, ax[t].x, o); ax[t].y += __shfl_xor_sync(0xffffffffu, ax[t].y, o);
+        ay[t].x += __shfl_xor_sync(0xffffffffu, ay[t].x, o); ay[t].y += __shfl_xor_sync(0xffffffffu, ay[t].y, o);
+        az[t].x += __shfl_xor_sync(0xffffffffu, az[t].x, o); az[t].y += __shfl_xor_sync(0xffffffffu, az[t].y, o);
+      }
+    }
+    if (lane >= 32 / S) return;
+  }
   // ---- fold the fp32 partial sums into the fp64 accumulators (sorted order)
 #pragma unroll
   for (int t = 0; t < TP; ++t) {
-    const uint32_t k0 = tgt_begin + t * 64 + lane, k1 = k0 + 32;
+    const uint32_t k0 = tgt_begin + t * (64 / S) + (lane & (32 / S - 1)), k1 = k0 + 32 / S;
     if (k0 < tgt_end) {
       red_add_f64(&acc64[3 * (size_t)k0 + 0], (double)ax[t].x);
       red_add_f64(&acc64[3 * (size_t)k0 + 1], (double)ay[t].x);
@@ -322,8 +341,8 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
     const uint32_t local = (uint32_t)(idx - __ldg(&item_prefix[c]));
     const uint32_t cs0 = __ldg(&cell_start[c]), cs1 = __ldg(&cell_start[c + 1]);
     const uint32_t n_c = cs1 - cs0;
-    const int T = targets_per_lane(n_c);
-    const uint32_t ntile = (n_c + 32u * T - 1) / (32u * T);
+    const uint32_t tpi = targets_per_item(n_c);
+    const uint32_t ntile = (n_c + tpi - 1) / tpi;
     const uint32_t tile = local % ntile, chunk = local / ntile;   // chunk-major: neighbours share sources
     const int cx = c % g.ncell[0], cy = (c / g.ncell[0]) % g.ncell[1], cz = c / (g.ncell[0] * g.ncell[1]);
 
@@ -357,11 +376,11 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
     __syncwarp();
 
     const uint32_t p0 = chunk * kSrcChunk, p1 = min(S, p0 + kSrcChunk);
-    const uint32_t tb = cs0 + tile * 32u * T, te = min(cs1, tb + 32u * T);
-    if (T == 2)
-      process_item<1, kUniformMass>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+    const uint32_t tb = cs0 + tile * tpi, te = min(cs1, tb + tpi);
+    if (n_c <= (uint32_t)kSmallCell)
+      process_item<1, kUniformMass, kSplit>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
     else
-      process_item<2, kUniformMass>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+      process_item<2, kUniformMass, 1>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
   }
 }
 
