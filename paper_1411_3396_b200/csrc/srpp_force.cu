@@ -63,16 +63,21 @@ __device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint
   return s;
 }
 
-// Targets of one work item.  Large cells: 32 lanes x 4 targets (two packed pairs per lane).  Cells of <= 64
-// particles (the uniform background: ~33 per cell) would leave half of a 64-target tile empty, so there the warp is
-// split 4 ways over the SOURCES: 8 lanes x 2 targets = 16 targets per item, lane group g = lane / 8 takes sources
-// g, g+4, g+8, ... of the staged tile, and the four partial sums are added with shuffles at the end.
-constexpr int kSmallCell = 64;
+// Targets of one work item.  Large cells: 32 lanes x 4 targets (two packed pairs per lane), several items per cell.
+// Cells of <= 48 particles (the uniform background: ~33 per cell) would leave half of a 64-target tile empty, so
+// there the warp is split 4 ways over the SOURCES: 8 lanes x 2 targets = 16 targets per packed pair, 1-3 packed
+// pairs per lane cover the WHOLE cell in one item (the staged sources are shared by all its targets), lane group
+// g = lane / 8 takes sources g, g+4, g+8, ... of the staged tile, and the four partial sums are added with shuffles
+// at the end.  Cells of 49..64 particles take one 64-target item.
 constexpr int kSplit = 4;                       // source phases of the small-cell path
-__device__ __forceinline__ uint32_t targets_per_item(uint32_t n_c) { return n_c <= (uint32_t)kSmallCell ? 64u / kSplit : 128u; }
+constexpr uint32_t kSplitMaxCell = 48;          // <= 3 packed pairs of 16 targets
+__device__ __forceinline__ uint32_t targets_per_item(uint32_t n_c, int fine) {
+  if (n_c <= kSplitMaxCell) return fine ? 16u : ((n_c + 15u) / 16u) * 16u;   // fine: tiny problems need more items
+  return n_c <= 64u ? 64u : 128u;
+}
 
 // ------------------------------------------------------------------- plan: items per cell, W, max --
-__global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__ cell_start, Geometry g,
+__global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__ cell_start, Geometry g, int fine,
                                                      unsigned long long* __restrict__ items, DevFlags* flags) {
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   unsigned long long w = 0, slots = 0;
@@ -89,7 +94,7 @@ __global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__
         const Segment s = stencil_segment(g, cell_start, cx, cy, cz, seg);
         S += s.end - s.start;
       }
-      const uint32_t tpi = targets_per_item(n_c);
+      const uint32_t tpi = targets_per_item(n_c, fine);
       const unsigned long long ntile = (n_c + tpi - 1) / tpi;
       const unsigned long long nchunk = (S + kSrcChunk - 1) / kSrcChunk;
       it = ntile * nchunk;
@@ -341,7 +346,7 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
     const uint32_t local = (uint32_t)(idx - __ldg(&item_prefix[c]));
     const uint32_t cs0 = __ldg(&cell_start[c]), cs1 = __ldg(&cell_start[c + 1]);
     const uint32_t n_c = cs1 - cs0;
-    const uint32_t tpi = targets_per_item(n_c);
+    const uint32_t tpi = targets_per_item(n_c, fc.fine_items);
     const uint32_t ntile = (n_c + tpi - 1) / tpi;
     const uint32_t tile = local % ntile, chunk = local / ntile;   // chunk-major: neighbours share sources
     const int cx = c % g.ncell[0], cy = (c / g.ncell[0]) % g.ncell[1], cz = c / (g.ncell[0] * g.ncell[1]);
@@ -377,8 +382,14 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
 
     const uint32_t p0 = chunk * kSrcChunk, p1 = min(S, p0 + kSrcChunk);
     const uint32_t tb = cs0 + tile * tpi, te = min(cs1, tb + tpi);
-    if (n_c <= (uint32_t)kSmallCell)
+    if (n_c <= 16u || (fc.fine_items && n_c <= kSplitMaxCell))
       process_item<1, kUniformMass, kSplit>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+    else if (n_c <= 32u)
+      process_item<2, kUniformMass, kSplit>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+    else if (n_c <= kSplitMaxCell)
+      process_item<3, kUniformMass, kSplit>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+    else if (n_c <= 64u)
+      process_item<1, kUniformMass, 1>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
     else
       process_item<2, kUniformMass, 1>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
   }
@@ -459,7 +470,8 @@ cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
   // reset queue head + statistics (keep the binning flags)
   if ((e = cudaMemsetAsync(&c->flags->max_cell_count, 0, sizeof(DevFlags) - offsetof(DevFlags, max_cell_count), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(c->acc64, 0, sizeof(double) * 3 * (size_t)n, st)) != cudaSuccess) return e;
-  k_plan_items<<<(ncells + 255) / 256, 256, 0, st>>>(c->cell_start, c->geo, c->item_prefix, c->flags);
+  c->fc.fine_items = n < (int64_t)c->num_sms * c->force_blocks_per_sm * kForceWarps * 64 ? 1 : 0;   // < 64 particles per resident warp
+  k_plan_items<<<(ncells + 255) / 256, 256, 0, st>>>(c->cell_start, c->geo, c->fc.fine_items, c->item_prefix, c->flags);
   const int nb = (ncells + kScanBlock - 1) / kScanBlock;
   k_scan_reduce<<<nb, kScanThreads, 0, st>>>(c->item_prefix, ncells, c->scan_tmp);
   k_scan_top<<<1, kScanThreads, 0, st>>>(c->scan_tmp, nb, &c->flags->total_items, &c->item_prefix[ncells]);

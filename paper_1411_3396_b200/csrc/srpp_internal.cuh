@@ -56,6 +56,7 @@ struct ForceConst {
   float eps2;            // eps^2 rounded to fp32: seeds the s-FMA chain, u = s + eps2
   float rc2e;            // rc^2 + eps2: cutoff test on u
   float nq[6];           // -Q(u) coefficients, Q(u) = P(u - eps2), expanded in fp64
+  int32_t fine_items;    // tiny problem: 16-target items so that every resident warp gets work
 };
 
 }  // namespace srpp
