@@ -95,6 +95,9 @@ def lib() -> C.CDLL:
         L.orc_kick.argtypes = [f32p, f32p, C.c_float, C.c_int64]
         L.orc_stream.restype = None
         L.orc_stream.argtypes = [f32p, f32p, C.c_float, f32p, C.c_int64]
+        L.orc_mbp.restype = None
+        L.orc_mbp.argtypes = [f32p, C.c_int64, C.POINTER(C.c_int64), C.c_int64, C.c_float, C.POINTER(C.c_double),
+                              C.POINTER(C.c_int64)]
         _lib = L
     return _lib
 
@@ -238,3 +241,17 @@ def error_norms(a_test, a_ref, allowance=None):
     tot = float(np.sum(ref * ref))
     glob = float(np.sqrt(np.sum(diff * diff) / tot)) if tot > 0 else float(np.sqrt(np.sum(diff * diff)))
     return per, glob
+
+
+def mbp(pos_mass, halo_start, eps: float):
+    """Most bound particle of every halo (reading R19).  halo_start: int64 [nhalo+1], halo h is the
+    run pos_mass[halo_start[h]:halo_start[h+1]].  Returns (phi f64 [n], index int64 [nhalo])."""
+    a, ap = _pm(pos_mass)
+    hs = np.ascontiguousarray(halo_start, dtype=np.int64)
+    nh = hs.shape[0] - 1
+    assert nh >= 0 and (nh == 0 or (hs[0] >= 0 and hs[-1] <= a.shape[0] and np.all(np.diff(hs) >= 0)))
+    phi = np.zeros(a.shape[0], dtype=np.float64)
+    idx = np.full(max(nh, 0), -1, dtype=np.int64)
+    lib().orc_mbp(ap, a.shape[0], hs.ctypes.data_as(C.POINTER(C.c_int64)), nh, C.c_float(eps),
+                  phi.ctypes.data_as(C.POINTER(C.c_double)), idx.ctypes.data_as(C.POINTER(C.c_int64)))
+    return phi, idx

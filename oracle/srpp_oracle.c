@@ -333,3 +333,41 @@ void orc_stream(float *pos_mass, const float *vel, float dt, const float *box, i
       pos_mass[4 * i + a] = y;
     }
 }
+
+/* ---------------------------------------------------------------- most bound particle (MBP) -- */
+/*
+ * Halo centre as the potential minimum, "most bound particle" (Sec. 2.2).
+ * The paper names the operation (its version is built from Thrust scan/transform/reduce) and prints no formula;
+ * the reading taken here (R19): for every member i of halo h = [halo_start[h], halo_start[h+1])
+ *
+ *     phi_i = - sum_{j in h, j != i}  m_j / sqrt(|x_j - x_i|^2 + eps^2)          (G = 1)
+ *
+ * with PLAIN coordinate differences (a halo finder hands over unwrapped members) and the Plummer softening of the
+ * force law (R3: -d/dr of -1/sqrt(r^2+eps^2) is the (s+eps^2)^(-3/2) term), and the centre is the member with the
+ * smallest phi, the lowest index winning ties.  An empty halo has index -1; a one-particle halo has phi = 0.
+ * phi[n] (fp64) and mbp[nhalo] (index into pos_mass) are outputs.  The plain definition, written out.
+ */
+void orc_mbp(const float *pos_mass, int64_t n, const int64_t *halo_start, int64_t nhalo, float eps, double *phi,
+             int64_t *mbp) {
+  (void)n;
+  const double e2 = (double)eps * (double)eps;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t h = 0; h < nhalo; ++h) {
+    const int64_t b = halo_start[h], e = halo_start[h + 1];
+    int64_t best = -1;
+    for (int64_t i = b; i < e; ++i) {
+      const double xi = pos_mass[4 * i], yi = pos_mass[4 * i + 1], zi = pos_mass[4 * i + 2];
+      double s = 0.0;
+      for (int64_t j = b; j < e; ++j) {
+        if (j == i) continue;
+        const double dx = (double)pos_mass[4 * j] - xi, dy = (double)pos_mass[4 * j + 1] - yi,
+                     dz = (double)pos_mass[4 * j + 2] - zi;
+        s += (double)pos_mass[4 * j + 3] / sqrt(dx * dx + dy * dy + dz * dz + e2);
+      }
+      phi[i] = -s;
+    }
+    for (int64_t i = b; i < e; ++i)
+      if (best < 0 || phi[i] < phi[best]) best = i;
+    mbp[h] = best;
+  }
+}

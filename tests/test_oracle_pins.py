@@ -388,3 +388,72 @@ def test_open_equals_periodic_when_no_pair_wraps(oracle_mod):
     a_per = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, 0.1))
     a_open = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, 0.1, periodic=(0, 0, 0)))
     assert np.array_equal(a_per, a_open)
+
+
+# --------------------------------------------------------- most bound particle (R19) --
+
+def test_mbp_closed_forms(oracle_mod):
+    """Two particles; N equal masses on a ring (all potentials equal, closed form); ring + centre particle."""
+    eps = float(np.float32(0.05))                        # eps crosses the interface as fp32, like srpp_params.eps
+    pos = np.array([[1.0, 2.0, 3.0, 2.0], [1.0, 2.0, 4.5, 3.0]], dtype=np.float32)
+    phi, idx = oracle_mod.mbp(pos, [0, 2], eps)
+    r = math.sqrt(1.5 ** 2 + eps ** 2)
+    assert phi[0] == pytest.approx(-3.0 / r, rel=1e-14) and phi[1] == pytest.approx(-2.0 / r, rel=1e-14)
+    assert idx[0] == 0                                   # the lighter particle sits deeper in the heavier one's well
+    n, R, m = 24, 5.0, 0.5
+    th = 2 * np.pi * np.arange(n) / n
+    ring = np.zeros((n + 1, 4), dtype=np.float32)
+    ring[:n, 0], ring[:n, 1], ring[:n, 2], ring[:, 3] = 40 + R * np.cos(th), 40 + R * np.sin(th), 7.0, m
+    ring[n, :3] = (40.0, 40.0, 7.0)
+    x = ring.astype(np.float64)
+    phi, idx = oracle_mod.mbp(ring, [0, n], eps)          # ring only
+    expect = [-m * sum(1.0 / math.sqrt(np.sum((x[k, :3] - x[i, :3]) ** 2) + eps ** 2) for k in range(n) if k != i)
+              for i in range(n)]
+    assert np.allclose(phi[:n], expect, rtol=1e-13)
+    chord = -m * sum(1.0 / math.sqrt((2 * R * math.sin(math.pi * k / n)) ** 2 + eps ** 2) for k in range(1, n))
+    assert np.allclose(phi[:n], chord, rtol=1e-6)         # fp32 ring coordinates: equal up to their rounding
+    phi, idx = oracle_mod.mbp(ring, [0, n + 1], eps)      # with the centre particle
+    assert idx[0] == n and phi[n] == pytest.approx(-n * m / math.sqrt(R * R + eps * eps), rel=1e-6)
+
+
+def test_mbp_halos_edge_cases_and_invariances(oracle_mod):
+    rng = np.random.default_rng(9)
+    pos, box = workloads.scaled_clustered(3000, (6, 6, 6), seed=4, frac_halo=1.0, n_halo=1, a_range=(1.0, 1.0))
+    hs = [0, 0, 1, 1200, 3000]                            # empty, single, two real halos
+    phi, idx = oracle_mod.mbp(pos, hs, 0.05)
+    assert idx[0] == -1 and idx[1] == 0 and phi[0] == 0.0
+    assert 1 <= idx[2] < 1200 and 1200 <= idx[3] < 3000
+    # independent numpy evaluation of one halo
+    x = pos[1200:3000].astype(np.float64)
+    d2 = ((x[:, None, :3] - x[None, :, :3]) ** 2).sum(-1) + float(np.float32(0.05)) ** 2
+    w = x[None, :, 3] / np.sqrt(d2)
+    np.fill_diagonal(w, 0.0)
+    assert np.allclose(phi[1200:3000], -w.sum(1), rtol=1e-12)
+    assert idx[3] == 1200 + int(np.argmin(-w.sum(1)))
+    # translation by a power of two is exact in fp32: same potentials, same centre
+    shifted = pos.copy()
+    shifted[:, :3] += np.float32(64.0)
+    phi2, idx2 = oracle_mod.mbp(shifted, hs, 0.05)
+    assert np.array_equal(idx, idx2) and np.allclose(phi, phi2, rtol=1e-6)
+    # permuting the members of a halo moves the centre with them
+    perm = rng.permutation(1800)
+    p2 = pos.copy()
+    p2[1200:3000] = pos[1200:3000][perm]
+    phi3, idx3 = oracle_mod.mbp(p2, hs, 0.05)
+    assert perm[idx3[3] - 1200] == idx[3] - 1200
+
+
+def test_mbp_plummer_centre(oracle_mod):
+    """A sampled Plummer sphere: the most bound particle lies well inside the scale radius of the true centre."""
+    rng = np.random.default_rng(3)
+    n, a = 4000, 1.5
+    u = rng.random(n) * (100.0 / 101.0) ** 1.5
+    r = a / np.sqrt(u ** (-2.0 / 3.0) - 1.0)
+    v = rng.normal(size=(n, 3))
+    v /= np.linalg.norm(v, axis=1)[:, None]
+    pos = np.ones((n, 4), dtype=np.float32)
+    pos[:, :3] = (50.0 + r[:, None] * v).astype(np.float32)
+    phi, idx = oracle_mod.mbp(pos, [0, n], 0.05)
+    assert np.linalg.norm(pos[idx[0], :3].astype(np.float64) - 50.0) < 0.3 * a
+    # potential depth of a Plummer sphere at its centre: -M/a (within sampling noise and truncation)
+    assert phi[idx[0]] == pytest.approx(-n / a, rel=0.1)
