@@ -412,8 +412,15 @@ def test_mbp_closed_forms(oracle_mod):
     assert np.allclose(phi[:n], expect, rtol=1e-13)
     chord = -m * sum(1.0 / math.sqrt((2 * R * math.sin(math.pi * k / n)) ** 2 + eps ** 2) for k in range(1, n))
     assert np.allclose(phi[:n], chord, rtol=1e-6)         # fp32 ring coordinates: equal up to their rounding
-    phi, idx = oracle_mod.mbp(ring, [0, n + 1], eps)      # with the centre particle
-    assert idx[0] == n and phi[n] == pytest.approx(-n * m / math.sqrt(R * R + eps * eps), rel=1e-6)
+    phi, idx = oracle_mod.mbp(ring, [0, n + 1], eps)      # with a particle at the centre
+    centre = -n * m / math.sqrt(R * R + eps * eps)
+    assert phi[n] == pytest.approx(centre, rel=1e-6)
+    assert np.allclose(phi[:n], chord - m / math.sqrt(R * R + eps * eps), rtol=1e-6)
+    assert chord - m / R < centre and idx[0] < n          # 24 close neighbours bind a ring member deeper than the centre
+    # a sparse ring (6 members): now the centre particle is the most bound one
+    hexa = np.concatenate([ring[0:n:4], ring[n:]])
+    phi, idx = oracle_mod.mbp(hexa, [0, 7], eps)
+    assert idx[0] == 6 and phi[6] == pytest.approx(-6 * m / math.sqrt(R * R + eps * eps), rel=1e-6)
 
 
 def test_mbp_halos_edge_cases_and_invariances(oracle_mod):
