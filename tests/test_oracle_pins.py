@@ -437,11 +437,11 @@ def test_mbp_halos_edge_cases_and_invariances(oracle_mod):
     np.fill_diagonal(w, 0.0)
     assert np.allclose(phi[1200:3000], -w.sum(1), rtol=1e-12)
     assert idx[3] == 1200 + int(np.argmin(-w.sum(1)))
-    # translation by a power of two is exact in fp32: same potentials, same centre
+    # translation invariance (the shifted fp32 coordinates are rounded, hence the tolerance)
     shifted = pos.copy()
     shifted[:, :3] += np.float32(64.0)
     phi2, idx2 = oracle_mod.mbp(shifted, hs, 0.05)
-    assert np.array_equal(idx, idx2) and np.allclose(phi, phi2, rtol=1e-6)
+    assert np.array_equal(idx, idx2) and np.allclose(phi, phi2, rtol=5e-5)
     # permuting the members of a halo moves the centre with them
     perm = rng.permutation(1800)
     p2 = pos.copy()
