@@ -142,6 +142,23 @@ int32_t srpp_probe_fp32(srpp_ctx* ctx, int32_t variant, int32_t trips, double* f
 int32_t srpp_set_boundary(srpp_ctx* ctx, const int32_t* periodic_host, const float* active_lo_host,
                           const float* active_hi_host);
 
+/* Most-bound-particle halo centre finder ("identification of the halo center as
+ * defined by its potential minimum (most bound particle)").  Reading R19: halo h is the contiguous run
+ * pos_mass[halo_start[h] .. halo_start[h+1]) and, for every member i,
+ *     phi_i = - sum_{j in h, j != i} m_j / sqrt(|x_j - x_i|^2 + eps^2)        (G = 1, eps of srpp_params, plain differences)
+ * The centre is the member with the smallest phi (lowest index on ties).
+ *   pos_mass          device float4[n]; positions need not lie in the box (no mesh is used)
+ *   halo_start_host   HOST int64[nhalo+1], non-decreasing, within [0, n]; read during the call
+ *   phi               device float[n] or NULL: phi of every halo member (entries outside every halo are not written)
+ *   mbp_index         device int64[nhalo]: index into pos_mass of each halo's centre, -1 for an empty halo
+ *   mbp_phi           device float[nhalo] or NULL: its potential (0 for an empty halo)
+ *   workspace         device, 256-byte aligned, >= srpp_mbp_workspace_bytes(n, nhalo); owned by the caller
+ * Pair arithmetic in fp32 (partial sums of <= 1024 terms folded in fp64).  Asynchronous on the context's stream after
+ * the halo table has been uploaded.  Errors: INVALID_ARG, WORKSPACE, CUDA. */
+int32_t srpp_mbp_workspace_bytes(int64_t n, int64_t nhalo, size_t* bytes_host);
+int32_t srpp_mbp(srpp_ctx* ctx, const float* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
+                 float* phi, int64_t* mbp_index, float* mbp_phi, void* workspace, size_t workspace_bytes);
+
 /* A7: sub-cycled kick, v <- fmaf(a, kdt, v) per component in fp32 (R16); .w lanes untouched.
  * vel, acc: device float4[n].  Asynchronous. */
 int32_t srpp_kick(srpp_ctx* ctx, float* vel, const float* acc, float kdt, int64_t n);

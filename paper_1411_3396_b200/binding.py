@@ -20,7 +20,7 @@ STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "GEOMETRY", -3: "DOMAIN", -4: "W
 EXPORTS = ("srpp_version", "srpp_default_poly", "srpp_workspace_bytes", "srpp_create", "srpp_destroy",
            "srpp_build_mesh", "srpp_get_mesh", "srpp_accel", "srpp_get_stats", "srpp_kick", "srpp_stream",
            "srpp_step_host", "srpp_strerror", "srpp_last_cuda_error", "srpp_set_timing", "srpp_get_timings",
-           "srpp_probe_fp32", "srpp_set_boundary")
+           "srpp_probe_fp32", "srpp_set_boundary", "srpp_mbp_workspace_bytes", "srpp_mbp")
 
 
 class SrppParams(C.Structure):
@@ -84,6 +84,10 @@ def load() -> C.CDLL:
     L.srpp_set_timing.argtypes = [vp, i32]
     L.srpp_get_timings.restype = i32
     L.srpp_get_timings.argtypes = [vp, C.POINTER(SrppTimings)]
+    L.srpp_mbp_workspace_bytes.restype = i32
+    L.srpp_mbp_workspace_bytes.argtypes = [i64, i64, C.POINTER(C.c_size_t)]
+    L.srpp_mbp.restype = i32
+    L.srpp_mbp.argtypes = [vp, vp, i64, C.POINTER(i64), i64, vp, vp, vp, vp, C.c_size_t]
     L.srpp_set_boundary.restype = i32
     L.srpp_set_boundary.argtypes = [vp, C.POINTER(i32), C.POINTER(C.c_float), C.POINTER(C.c_float)]
     L.srpp_probe_fp32.restype = i32
@@ -233,6 +237,25 @@ class Solver:
         t = SrppTimings()
         self._check(self.lib.srpp_get_timings(self._ctx, C.byref(t)), "srpp_get_timings")
         return {k: float(getattr(t, k)) for k, _ in SrppTimings._fields_}
+
+    def mbp(self, pos_mass, halo_start, want_phi: bool = True):
+        """srpp_mbp: most bound particle of every halo.  halo_start: host int64 sequence [nhalo+1].
+        Returns (index int64 [nhalo], phi_min float32 [nhalo], phi float32 [n] or None), device tensors."""
+        import numpy as np
+        torch = self._torch
+        hs = np.ascontiguousarray(halo_start, dtype=np.int64)
+        nh, n = int(hs.shape[0]) - 1, int(pos_mass.shape[0])
+        nbytes = C.c_size_t(0)
+        self._check(self.lib.srpp_mbp_workspace_bytes(n, nh, C.byref(nbytes)), "srpp_mbp_workspace_bytes")
+        ws = torch.empty(max(int(nbytes.value), 256), dtype=torch.uint8, device=self.device)
+        idx = torch.empty(max(nh, 1), dtype=torch.int64, device=self.device)[:nh]
+        pmin = torch.empty(max(nh, 1), dtype=torch.float32, device=self.device)[:nh]
+        phi = torch.zeros(max(n, 1), dtype=torch.float32, device=self.device)[:n] if want_phi else None
+        self._check(self.lib.srpp_mbp(self._ctx, pos_mass.data_ptr(), n, hs.ctypes.data_as(C.POINTER(C.c_int64)), nh,
+                                      phi.data_ptr() if want_phi else None, idx.data_ptr(), pmin.data_ptr(),
+                                      ws.data_ptr(), int(nbytes.value)), "srpp_mbp")
+        self._mbp_ws = ws                                  # keep the workspace alive until the stream has run
+        return idx, pmin, phi
 
     def set_boundary(self, periodic=(1, 1, 1), active_lo=None, active_hi=None) -> None:
         """srpp_set_boundary: open (non-periodic) axes and the active box of an overloaded node volume."""

@@ -245,6 +245,28 @@ int32_t srpp_set_boundary(srpp_ctx* c, const int32_t* periodic_host, const float
   return SRPP_OK;
 }
 
+int32_t srpp_mbp_workspace_bytes(int64_t n, int64_t nhalo, size_t* bytes_host) {
+  if (!bytes_host || n < 0 || n >= ((int64_t)1 << 31) || nhalo < 0 || nhalo >= ((int64_t)1 << 31)) return SRPP_ERR_INVALID_ARG;
+  size_t a, b, d;
+  *bytes_host = mbp_workspace_layout(n, nhalo, &a, &b, &d);
+  return SRPP_OK;
+}
+
+int32_t srpp_mbp(srpp_ctx* c, const float* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
+                 float* phi, int64_t* mbp_index, float* mbp_phi, void* workspace, size_t workspace_bytes) {
+  if (!c || n < 0 || n >= ((int64_t)1 << 31) || nhalo < 0 || nhalo >= ((int64_t)1 << 31) || !halo_start_host ||
+      (n > 0 && !pos_mass) || (nhalo > 0 && !mbp_index) || !workspace)
+    return SRPP_ERR_INVALID_ARG;
+  if (halo_start_host[0] < 0 || halo_start_host[nhalo] > n) return SRPP_ERR_INVALID_ARG;
+  for (int64_t h = 0; h < nhalo; ++h)
+    if (halo_start_host[h + 1] < halo_start_host[h]) return SRPP_ERR_INVALID_ARG;
+  size_t a, b, d;
+  if (((uintptr_t)workspace & 255u) != 0 || workspace_bytes < mbp_workspace_layout(n, nhalo, &a, &b, &d)) return SRPP_ERR_WORKSPACE;
+  const cudaError_t e = launch_mbp(c, (const float4*)pos_mass, n, halo_start_host, nhalo, phi, (long long*)mbp_index,
+                                   mbp_phi, (char*)workspace);
+  return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
+}
+
 int32_t srpp_build_mesh(srpp_ctx* c, const float* pos_mass, int64_t n) {
   if (!c || n < 0 || n >= ((int64_t)1 << 31) || (n > 0 && !pos_mass)) return SRPP_ERR_INVALID_ARG;
   c->n = -1;

@@ -103,6 +103,7 @@ struct srpp_ctx {
   cudaEvent_t ev[srpp::kNumEvents];
   bool ev_mesh_valid, ev_accel_valid;
   uint64_t launches;         // kernels launched by this context so far (harness evidence)
+  unsigned long long mbp_pairs;  // sum of n_h^2 of the last srpp_mbp call (ordered pairs incl. self, the metric's unit)
 };
 
 namespace srpp {
@@ -117,6 +118,10 @@ cudaError_t launch_accel(srpp_ctx* c, float4* acc);
 cudaError_t launch_kick(srpp_ctx* c, float4* vel, const float4* acc, float kdt, int64_t n);
 cudaError_t launch_stream(srpp_ctx* c, float4* pos_mass, const float4* vel, float dt, int64_t n);
 int query_force_occupancy();
+// srpp_mbp.cu
+size_t mbp_workspace_layout(int64_t n, int64_t nhalo, size_t* o_phi, size_t* o_prefix, size_t* o_start);
+cudaError_t launch_mbp(srpp_ctx* c, const float4* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
+                       float* phi_out, long long* mbp_index, float* mbp_phi, char* ws);
 // srpp_probe.cu
 cudaError_t run_fp32_probe(cudaStream_t st, int variant, int iters, double* flops_per_s, float* checksum);
 

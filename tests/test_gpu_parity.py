@@ -439,3 +439,62 @@ def test_overloaded_subvolume_reproduces_periodic_box(oracle_mod, gpu):
     # the shifted coordinates differ from the originals by an fp32 rounding, so allow twice the usual global bar
     per, glob = oracle_mod.error_norms(a[active_sub], ref, st["allowance"])
     assert per.max() <= PER_PARTICLE_TOL and glob <= 2 * GLOBAL_L2_TOL, (per.max(), glob)
+
+
+# --------------------------------------------------------------- most bound particle --
+
+def _mbp_check(oracle_mod, gpu, pos, hs, eps):
+    torch, binding = gpu
+    sol = binding.Solver((64.0,) * 3, (10,) * 3, 3.0, eps, n_max=16)
+    d = torch.from_numpy(np.ascontiguousarray(pos)).cuda()
+    idx, pmin, phi = sol.mbp(d, hs)
+    torch.cuda.synchronize()
+    idx, pmin, phi = idx.cpu().numpy(), pmin.cpu().numpy(), phi.cpu().numpy()
+    o_phi, o_idx = oracle_mod.mbp(pos, hs, eps)
+    hs = np.asarray(hs, dtype=np.int64)
+    member = np.zeros(pos.shape[0], dtype=bool)
+    for h in range(len(hs) - 1):
+        member[hs[h]:hs[h + 1]] = True
+    # potentials: fp32 pair terms, <= 1024-term partial sums folded in fp64 -> 1e-5 relative to the halo's depth
+    scale = np.maximum(np.abs(o_phi), 1e-30)
+    assert np.all(np.abs(phi[member] - o_phi[member]) <= 2e-5 * scale[member] + 1e-6)
+    for h in range(len(hs) - 1):
+        if hs[h + 1] == hs[h]:
+            assert idx[h] == -1 and pmin[h] == 0.0
+            continue
+        assert hs[h] <= idx[h] < hs[h + 1]
+        # the argmin is decided in fp32 on the GPU: its choice must be a minimum of the fp64 potential up to that error
+        assert o_phi[idx[h]] <= o_phi[o_idx[h]] * (1 - 4e-5) + 1e-6
+        assert abs(pmin[h] - o_phi[o_idx[h]]) <= 4e-5 * abs(o_phi[o_idx[h]]) + 1e-6
+    return idx, o_idx
+
+
+def test_mbp_small_halos_and_edge_cases(oracle_mod, gpu):
+    rng = np.random.default_rng(12)
+    pos, box = workloads.scaled_clustered(30000, (8, 8, 8), seed=12, frac_halo=1.0, n_halo=6, a_range=(0.3, 1.5))
+    pos[:, 3] = rng.uniform(0.5, 1.5, pos.shape[0]).astype(np.float32)
+    cuts = np.sort(rng.choice(np.arange(2, 29000), 60, replace=False))
+    hs = np.concatenate([[0, 0, 1], cuts, [29000, 29000]])      # empty, single, ragged sizes; tail not in a halo
+    idx, o_idx = _mbp_check(oracle_mod, gpu, pos, hs, 0.05)
+    assert (idx == o_idx).mean() > 0.9
+
+
+def test_mbp_plummer_halos(oracle_mod, gpu):
+    """Halos as the workload generator makes them (one Plummer sphere each, equal masses), sizes 40 ... 60000:
+    spans one to many target tiles and source chunks."""
+    rng = np.random.default_rng(5)
+    sizes = [40, 127, 128, 129, 1024, 1025, 5000, 60000]
+    parts, hs = [], [0]
+    for k, n in enumerate(sizes):
+        a = 0.5 + 0.3 * k
+        u = rng.random(n) * (100.0 / 101.0) ** 1.5
+        r = a / np.sqrt(u ** (-2.0 / 3.0) - 1.0)
+        v = rng.normal(size=(n, 3))
+        v /= np.linalg.norm(v, axis=1)[:, None]
+        p = np.ones((n, 4), dtype=np.float32)
+        p[:, :3] = (rng.uniform(20, 200, 3) + r[:, None] * v).astype(np.float32)
+        parts.append(p)
+        hs.append(hs[-1] + n)
+    pos = np.concatenate(parts)
+    idx, o_idx = _mbp_check(oracle_mod, gpu, pos, hs, 0.05)
+    assert np.array_equal(idx, o_idx)
