@@ -17,8 +17,9 @@ constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortItems = 8;                 // a warp handles 8 steps of 32 consecutive elements
 constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 elements per tile
 constexpr int kSortMinDigitBits = 5;          // >= 32 bins (one warp-row of the column scan)
-constexpr int kSortMaxDigitBits = 10;         // <= 1024 bins (>= 4 elements per bin and tile): two passes cover 2^20 cells
+constexpr int kSortMaxDigitBits = 8;          // <= 256 bins: >= 16 elements per bin and tile, so the per-digit runs cover whole 32-byte sectors
 constexpr int kSortMaxBins = 1 << kSortMaxDigitBits;
+constexpr int kSortBinsPerThread = kSortMaxBins > kSortThreads ? kSortMaxBins / kSortThreads : 1;
 
 constexpr int kForceThreads = 256;            // 8 autonomous warps per CTA
 constexpr int kForceWarps = kForceThreads / 32;

@@ -4,7 +4,7 @@
 //   A1  cell id per particle, fp32:  c = min((int)floorf(x * inv), ncell-1), inv = (float)ncell/box
 //   A2-A4 histogram / exclusive scan / stable scatter.  A cell id has up to 24 bits and single cells hold
 //        millions of particles, so the counting sort is applied digit-wise, least significant digit first,
-//        with WIDE digits (<= 10 bits: two passes cover 2^20 cells, three 2^24) and with the particle PAYLOAD
+//        in digits of <= 8 bits (three passes cover the 2^24-cell limit) and with the particle PAYLOAD
 //        (float4 position+mass and original index) carried through every pass.  All global traffic is
 //        streaming: each pass reads its input once, coalesced, re-orders a 4096-element tile by digit in
 //        shared memory, and writes per-digit runs.  No random gather remains (the first version sorted
@@ -14,8 +14,10 @@
 //        counting sort.
 //   cell_start = run boundaries of the sorted ids (= exclusive prefix sum of the cell histogram).
 // Per pass: [per-tile digit histogram (fused into A1 for the first pass)] -> column scan over tiles ->
-// scatter.  Algorithmic bytes per build: 52*N + 8*ncells; moved by this design for two
-// passes: 20 + 44 + 4 + 48 + 4 = 120 bytes per particle, all coalesced.
+// scatter.  Algorithmic bytes per build: 52*N + 8*ncells; moved by this design for three
+// passes: 20 + 44 + 4 + 48 + 4 + 48 + 4 = 172 bytes per particle, all coalesced.  (Two passes of 10-bit digits move
+// 120 bytes, but a 4096-element tile then writes 4-element runs per digit: the partially covered 32-byte sectors cost
+// more DRAM read-modify-write traffic than the third pass -- measured.)
 // Paper context: PAPER.md:63/65 (direct PP short-range solver inside the hand-over radius); the chaining
 // mesh itself is named by BASELINE.json north_star.
 #include <algorithm>
@@ -54,15 +56,15 @@ __device__ __forceinline__ uint32_t cta_exclusive_scan(uint32_t v, uint32_t* scr
 __device__ __forceinline__ void cta_scan_bins(uint32_t* a, int nbins, uint32_t* scratch) {
   const int per = nbins > kSortThreads ? nbins / kSortThreads : 1;   // 1, 2 or 4
   const int b0 = threadIdx.x * per;
-  uint32_t v[kSortMaxBins / kSortThreads], s = 0;
+  uint32_t v[kSortBinsPerThread], s = 0;
 #pragma unroll
-  for (int j = 0; j < kSortMaxBins / kSortThreads; ++j) {
+  for (int j = 0; j < kSortBinsPerThread; ++j) {
     v[j] = (j < per && b0 + j < nbins) ? a[b0 + j] : 0u;
     s += v[j];
   }
   uint32_t ex = cta_exclusive_scan(s, scratch);
 #pragma unroll
-  for (int j = 0; j < kSortMaxBins / kSortThreads; ++j) {
+  for (int j = 0; j < kSortBinsPerThread; ++j) {
     if (j < per && b0 + j < nbins) a[b0 + j] = ex;
     ex += v[j];
   }
@@ -309,9 +311,9 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_digit_scatter(
   for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
     const int64_t tile = t * kSortTile;
     const int tile_n = (int)min((int64_t)kSortTile, n - tile);
-    uint32_t goff[kSortMaxBins / kSortThreads];      // first: elements of the digit in earlier tiles
+    uint32_t goff[kSortBinsPerThread];      // first: elements of the digit in earlier tiles
 #pragma unroll
-    for (int j = 0; j < kSortMaxBins / kSortThreads; ++j) {
+    for (int j = 0; j < kSortBinsPerThread; ++j) {
       const int d = threadIdx.x + j * kSortThreads;
       goff[j] = d < nbins ? __ldg(&hist[(size_t)t * nbins + d]) : 0u;
     }
@@ -339,15 +341,20 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_digit_scatter(
     }
     __syncthreads();
     // ---- per digit: exclusive prefix over the warps; tile count of the digit -> tstart (scanned next)
-    for (int d = threadIdx.x; d < nbins; d += kSortThreads) {
-      uint32_t run = 0;
+    {   // two adjacent digits per thread: one 32-bit access carries both u16 counters (counts <= 4096: no carry)
+      uint32_t* wc32 = (uint32_t*)wc;
+      const int half = nbins >> 1;
+      for (int dp = threadIdx.x; dp < half; dp += kSortThreads) {
+        uint32_t run = 0;
 #pragma unroll
-      for (int r = 0; r < kSortWarps; ++r) {
-        const uint32_t c = wc[(size_t)r * nbins + d];
-        wc[(size_t)r * nbins + d] = (unsigned short)run;
-        run += c;
+        for (int r = 0; r < kSortWarps; ++r) {
+          const uint32_t c = wc32[(size_t)r * half + dp];
+          wc32[(size_t)r * half + dp] = run;
+          run += c;
+        }
+        tstart[2 * dp] = run & 0xffffu;
+        tstart[2 * dp + 1] = run >> 16;
       }
-      tstart[d] = run;
     }
     __syncthreads();
     cta_scan_bins(tstart, nbins, scratch);
@@ -359,7 +366,7 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_digit_scatter(
     }
     // goff[d] = (start of the digit + elements of the digit in earlier tiles) - its start inside this tile
 #pragma unroll
-    for (int j = 0; j < kSortMaxBins / kSortThreads; ++j) {
+    for (int j = 0; j < kSortBinsPerThread; ++j) {
       const int d = threadIdx.x + j * kSortThreads;
       if (d < nbins) goff[j] += base[d] - tstart[d];
     }
@@ -376,7 +383,7 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_digit_scatter(
       }
     }
 #pragma unroll
-    for (int j = 0; j < kSortMaxBins / kSortThreads; ++j) {
+    for (int j = 0; j < kSortBinsPerThread; ++j) {
       const int d = threadIdx.x + j * kSortThreads;
       if (d < nbins) tstart[d] = goff[j];
     }
@@ -433,7 +440,7 @@ __global__ void __launch_bounds__(256) k_cell_start(const uint32_t* __restrict__
 }
 
 // ------------------------------------------------------------------------------------ host launcher --
-// Digit plan: the cell id has `bits` significant bits; passes = ceil(bits / 10), digits of equal width.
+// Digit plan: the cell id has `bits` significant bits; passes = ceil(bits / 8), digits of equal width.
 void plan_sort(int32_t ncells, int* passes, int* digit_bits) {
   int bits = kSortMinDigitBits;
   while (((int64_t)1 << bits) < (int64_t)ncells) ++bits;

@@ -101,18 +101,19 @@ def test_binning_uniform_ragged_sizes(oracle_mod, gpu, n):
     _check_mesh(oracle_mod, gpu, pos, box, ncell)
 
 
-@pytest.mark.parametrize("ncell,n", [((100, 100, 100), 300000),     # 1,000,000 cells: 20 bits -> 2 digits of 10
+@pytest.mark.parametrize("ncell,n", [((100, 100, 100), 300000),     # 1,000,000 cells: 20 bits -> 3 digits of 7
                                      ((160, 160, 160), 300000),     # 4,096,000 cells: 22 bits -> 3 digits of 8
                                      ((256, 256, 256), 200000),     # 2^24 cells (the maximum): 3 digits of 8
+                                     ((40, 40, 40), 200000),        # 64,000 cells: 16 bits -> 2 digits of 8
                                      ((3, 3, 3), 5000)])            # 27 cells: one digit of 5 bits
 def test_binning_digit_plans(oracle_mod, gpu, ncell, n):
-    """Every digit plan of the LSD counting sort (1, 2 and 3 passes; 32 ... 1024 bins), clustered input."""
+    """Every digit plan of the LSD counting sort (1, 2 and 3 passes; 32 ... 256 bins), clustered input."""
     pos, box = workloads.scaled_clustered(n, ncell, seed=5, frac_halo=0.7, n_halo=30, a_range=(0.2, 2.0))
     _check_mesh(oracle_mod, gpu, pos, box, ncell)
 
 
 def test_binning_two_digits_clustered(oracle_mod, gpu):
-    """84,480 cells (two 9-bit digits), heavy cells, empty cells, random memory order."""
+    """84,480 cells (17 bits: three 6-bit digits), heavy cells, empty cells, random memory order."""
     ncell = (48, 40, 44)
     pos, box = workloads.scaled_clustered(600000, ncell, seed=21, frac_halo=0.8, n_halo=40, a_range=(0.2, 2.0))
     sol = _check_mesh(oracle_mod, gpu, pos, box, ncell)
