@@ -11,7 +11,7 @@
 namespace srpp {
 
 // ---- tunables ------------------------------------------------------------------------------
-// binning: LSD counting sort of the cell id in wide digits, payload carried (srpp_mesh.cu)
+// binning: LSD counting sort of the cell id in digits of <= 8 bits, payload carried (srpp_mesh.cu)
 constexpr int kSortThreads = 512;             // 16 warps
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortItems = 8;                 // a warp handles 8 steps of 32 consecutive elements
@@ -23,7 +23,7 @@ constexpr int kSortBinsPerThread = kSortMaxBins > kSortThreads ? kSortMaxBins / 
 
 constexpr int kForceThreads = 256;            // 8 autonomous warps per CTA
 constexpr int kForceWarps = kForceThreads / 32;
-constexpr int kSrcTile = 128;                 // sources staged per warp-private smem tile (64 pairs)
+constexpr int kSrcTile = 128;                 // sources staged per warp-private smem tile (float4 each)
 constexpr int kSrcChunk = 1024;               // sources per work item (fp32 partial-sum length)
 constexpr int kMaxSeg = 18;                   // 9 (dy,dz) rows x up to 2 x-segments (periodic wrap)
 
