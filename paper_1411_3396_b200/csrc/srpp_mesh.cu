@@ -134,24 +134,44 @@ __global__ void __launch_bounds__(kSortThreads) k_keys_hist(const float4* __rest
 // ------------------------------------------------------ A2 (later digits): per-tile digit histogram --
 __global__ void __launch_bounds__(kSortThreads) k_digit_hist(const uint32_t* __restrict__ keys, int64_t n, int shift,
                                                               int nbins, uint32_t* __restrict__ hist, int64_t ntiles) {
-  extern __shared__ uint32_t h_dyn[];
+  extern __shared__ uint32_t h_dyn[];                  // two histograms: tiles alternate, one barrier per tile
   const uint32_t mask = (uint32_t)nbins - 1u;
-  for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
-    for (int d = threadIdx.x; d < nbins; d += kSortThreads) h_dyn[d] = 0u;
-    __syncthreads();
-    const int64_t beg = t * kSortTile, end = min(n, beg + kSortTile);
-    uint32_t k[kSortItems];
+  uint32_t k[kSortItems];
+  {
+    const int64_t beg = (int64_t)blockIdx.x * kSortTile;
 #pragma unroll
     for (int u = 0; u < kSortItems; ++u) {
       const int64_t i = beg + threadIdx.x + u * kSortThreads;
-      k[u] = i < end ? __ldg(&keys[i]) : 0u;
+      k[u] = i < n ? __ldcs(&keys[i]) : 0u;
+    }
+  }
+  for (int d = threadIdx.x; d < 2 * nbins; d += kSortThreads) h_dyn[d] = 0u;
+  __syncthreads();
+  int buf = 0;
+  for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x, buf ^= 1) {
+    uint32_t* h = h_dyn + buf * nbins;
+    const int64_t beg = t * kSortTile, end = min(n, beg + kSortTile);
+    uint32_t cur[kSortItems];
+#pragma unroll
+    for (int u = 0; u < kSortItems; ++u) cur[u] = k[u];
+    // next tile's keys are in flight while this tile is counted
+    {
+      const int64_t nbeg = (t + gridDim.x) * kSortTile;
+#pragma unroll
+      for (int u = 0; u < kSortItems; ++u) {
+        const int64_t i = nbeg + threadIdx.x + u * kSortThreads;
+        k[u] = i < n ? __ldcs(&keys[i]) : 0u;
+      }
     }
 #pragma unroll
     for (int u = 0; u < kSortItems; ++u)
-      hist_add(h_dyn, (k[u] >> shift) & mask, beg + threadIdx.x + u * kSortThreads < end);
+      hist_add(h, (cur[u] >> shift) & mask, beg + threadIdx.x + u * kSortThreads < end);
     __syncthreads();
-    for (int d = threadIdx.x; d < nbins; d += kSortThreads) hist[(size_t)t * nbins + d] = h_dyn[d];
-    __syncthreads();
+    // write this tile's row and clear the buffer for the tile after next (the other buffer is already clear)
+    for (int d = threadIdx.x; d < nbins; d += kSortThreads) {
+      hist[(size_t)t * nbins + d] = h[d];
+      h[d] = 0u;
+    }
   }
 }
 
@@ -488,7 +508,7 @@ cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n) {
   for (int p = 0; p < passes; ++p) {
     const int shift = p * dbits;
     const int o = p & 1;
-    if (p > 0) k_digit_hist<<<hblocks, kSortThreads, smem_hist, st>>>(kin, n, shift, nbins, c->hist, tiles);
+    if (p > 0) k_digit_hist<<<hblocks, kSortThreads, 2 * smem_hist, st>>>(kin, n, shift, nbins, c->hist, tiles);
     k_col_sum<<<dim3(nbins / 32, kScanSlices), 1024, 0, st>>>(c->hist, tiles, nbins, c->colpart);
     k_col_scan<<<dim3(nbins / 32, kScanSlices), 1024, 0, st>>>(c->hist, tiles, nbins, c->colpart, c->coltot);
     if (p == 0)
