@@ -499,3 +499,32 @@ def test_mbp_plummer_halos(oracle_mod, gpu):
     pos = np.concatenate(parts)
     idx, o_idx = _mbp_check(oracle_mod, gpu, pos, hs, 0.05)
     assert np.array_equal(idx, o_idx)
+
+
+def test_new_entry_points_reject_bad_arguments(gpu):
+    """Error behaviour stated in include/srpp.h for srpp_set_boundary and srpp_mbp."""
+    import ctypes as C
+    torch, binding = gpu
+    sol = binding.Solver((32.0,) * 3, (10,) * 3, 3.0, 0.1, n_max=100)
+    with pytest.raises(binding.SrppError) as e:
+        sol.set_boundary((1, 1, 1), (5.0, 0.0, 0.0), (4.0, 32.0, 32.0))       # lo > hi
+    assert e.value.status == -1
+    with pytest.raises(binding.SrppError) as e:
+        sol.set_boundary((1, 1, 1), (float("nan"), 0.0, 0.0), (4.0, 32.0, 32.0))
+    assert e.value.status == -1
+    pos = torch.rand((100, 4), device="cuda")
+    with pytest.raises(binding.SrppError) as e:
+        sol.mbp(pos, [0, 60, 40, 100])                                        # not monotone
+    assert e.value.status == -1
+    with pytest.raises(binding.SrppError) as e:
+        sol.mbp(pos, [0, 101])                                                # beyond n
+    assert e.value.status == -1
+    hs = (C.c_int64 * 2)(0, 100)
+    idx = torch.empty(1, dtype=torch.int64, device="cuda")
+    ws = torch.empty(512, dtype=torch.uint8, device="cuda")
+    rc = sol.lib.srpp_mbp(sol._ctx, pos.data_ptr(), 100, hs, 1, None, idx.data_ptr(), None, ws.data_ptr(), 512)
+    assert rc == -4                                                           # workspace too small
+    # a valid call still works afterwards
+    i, p, phi = sol.mbp(pos, [0, 100])
+    torch.cuda.synchronize()
+    assert 0 <= int(i[0]) < 100
