@@ -16,7 +16,10 @@ Pins (tests/test_oracle_pins.py): P1 two-particle closed form, P2 zero beyond
 the cutoff, P3 unit lattice (122 neighbours, zero net force), P4 momentum
 conservation, P5 8-particle worked example, P6 brute force vs cell list,
 P7 config-1 soft pins, P8 binning worked example, P9/P10 coefficient table,
-P11 permutation invariance.  Unpinned: fidelity of the DEFAULT polynomial to
+P11 permutation invariance; the R9 allowance band (constructed near-cutoff
+neighbours), the R18 metric (hand-computed vectors) and the sub-cycle
+`orc_subcycle` (two-particle step worked by hand from P1's printed values,
+composition, momentum, time reversal).  Unpinned: fidelity of the DEFAULT polynomial to
 the real HACC grid force ("parity unpinned": PAPER.md prints nothing to
 compare with; both sides take poly[6] as data, so GPU-vs-oracle parity does
 not depend on it).
@@ -95,6 +98,8 @@ def lib() -> C.CDLL:
         L.orc_kick.argtypes = [f32p, f32p, C.c_float, C.c_int64]
         L.orc_stream.restype = None
         L.orc_stream.argtypes = [f32p, f32p, C.c_float, f32p, C.c_int64]
+        L.orc_subcycle.restype = C.c_int32
+        L.orc_subcycle.argtypes = [f32p, f32p, C.c_int64, C.POINTER(Params), C.c_float, C.c_float, C.c_int32, f32p]
         L.orc_mbp.restype = None
         L.orc_mbp.argtypes = [f32p, C.c_int64, C.POINTER(C.c_int64), C.c_int64, C.c_float, C.POINTER(C.c_double),
                               C.POINTER(C.c_int64)]
@@ -219,6 +224,21 @@ def stream(pos_mass, vel, dt: float, box) -> np.ndarray:
     b, bp = _f32(box)
     lib().orc_stream(x.ctypes.data_as(C.POINTER(C.c_float)), vp, float(dt), bp, x.shape[0])
     return x
+
+
+def subcycle(pos_mass, vel, params: Params, dt: float, kdt: float, nsub: int = 1):
+    """nsub x { stream(dt/2); a = accel (fp64 sum rounded once to fp32); kick(kdt); stream(dt/2) } (R20).
+    Returns new (pos_mass, vel, acc) as float32 [n,4] arrays; acc = accelerations of the last sub-step."""
+    x = np.array(pos_mass, dtype=np.float32, order="C", copy=True)
+    v = np.array(vel, dtype=np.float32, order="C", copy=True)
+    assert x.ndim == 2 and x.shape[1] == 4 and v.shape == x.shape
+    a = np.zeros_like(x)
+    f32p = C.POINTER(C.c_float)
+    rc = lib().orc_subcycle(x.ctypes.data_as(f32p), v.ctypes.data_as(f32p), x.shape[0], C.byref(params),
+                            C.c_float(dt), C.c_float(kdt), int(nsub), a.ctypes.data_as(f32p))
+    if rc != 0:
+        raise MemoryError("oracle subcycle failed (%d)" % rc)
+    return x, v, a
 
 
 def error_norms(a_test, a_ref, allowance=None):

@@ -371,3 +371,37 @@ void orc_mbp(const float *pos_mass, int64_t n, const int64_t *halo_start, int64_
     mbp[h] = best;
   }
 }
+
+/* ---------------------------------------------------------------- short-range sub-cycle -- */
+/*
+ * The "short-range force timestep" of PAPER.md:73 (Sec. 2.1: every block is evolved, its active particles updated,
+ * the passive ones only streamed) as one call.  PAPER.md does not print the integrator; the reading taken here
+ * (R20; SURVEY.md 8(f) item 1 "stream-kick-stream", R16, R17) is the symmetric split
+ *
+ *     repeat nsub times:   x <- stream(x, v, dt/2);   a = accel(x);   v <- kick(v, a, kdt);   x <- stream(x, v, dt/2)
+ *
+ * written out with the pieces above and nothing else: orc_stream (fp32 fma + wrap, R13/R17), the fp64 cell-list sum
+ * orc_accel rounded ONCE to fp32 (the kick is an fp32 operation on fp32 accelerations, R16), orc_kick.  dt/2 is the
+ * fp32 product 0.5f*dt (exact).  pos_mass[4n], vel[4n] are updated in place; acc[4n] (may be NULL) receives the fp32
+ * accelerations of the LAST sub-step, .w = 0.  Returns 0, or -6 if out of memory.
+ */
+int32_t orc_subcycle(float *pos_mass, float *vel, int64_t n, const orc_params *p, float dt, float kdt, int32_t nsub,
+                     float *acc) {
+  double *a64 = (double *)malloc(sizeof(double) * 3 * (size_t)(n > 0 ? n : 1));
+  float *a32 = (float *)calloc(4 * (size_t)(n > 0 ? n : 1), sizeof(float));
+  if (!a64 || !a32) { free(a64); free(a32); return -6; }
+  const float half = 0.5f * dt;
+  for (int32_t s = 0; s < nsub; ++s) {
+    orc_stream(pos_mass, vel, half, p->box, n);
+    int32_t rc = orc_accel(pos_mass, n, p, NULL, n, a64, NULL, NULL, NULL, NULL);
+    if (rc != 0) { free(a64); free(a32); return rc; }
+    for (int64_t i = 0; i < n; ++i)
+      for (int a = 0; a < 3; ++a) a32[4 * i + a] = (float)a64[3 * i + a];
+    orc_kick(vel, a32, kdt, n);
+    orc_stream(pos_mass, vel, half, p->box, n);
+  }
+  if (acc) memcpy(acc, a32, sizeof(float) * 4 * (size_t)n);
+  free(a64);
+  free(a32);
+  return 0;
+}

@@ -464,3 +464,172 @@ def test_mbp_plummer_centre(oracle_mod):
     assert np.linalg.norm(pos[idx[0], :3].astype(np.float64) - 50.0) < 0.3 * a
     # potential depth of a Plummer sphere at its centre: -M/a (within sampling noise and truncation)
     assert phi[idx[0]] == pytest.approx(-n / a, rel=0.1)
+
+
+# --------------------------------------------------------- R9 allowance and the R18 metric (the checker's own pins) --
+
+def _independent_factor(s, eps32):
+    """f(s) = (s + eps^2)^(-3/2) - P(s) typed out once more in numpy fp64 (np.polyval on the printed coefficients)."""
+    c = np.array([fnum(r[1]) for r in golden_lines("poly_default.txt")], dtype=np.float32).astype(np.float64)
+    return (s + float(eps32) ** 2) ** -1.5 - np.polynomial.polynomial.polyval(s, c)
+
+
+def test_r9_allowance_band(oracle_mod):
+    """R9: the allowance of a target is sum |m_j f d| over pairs with |s - rc^2| <= 2^-18 rc^2, taken as if inside the
+    cutoff, and nothing else.  Target at (1,1,1); neighbour A two ulps inside rc along x (|s-9|/9 ~ 2^-21.6: in the
+    band), neighbour B at relative distance ~2^-16 from rc^2 along y (outside the band, inside the cutoff), neighbour C
+    two ulps OUTSIDE rc along z (in the band, contributes to the allowance but not to the force), D far inside."""
+    eps = np.float32(0.1)
+    one, four = np.float32(1.0), np.float32(4.0)
+    xa = np.nextafter(np.nextafter(four, np.float32(0)), np.float32(0))            # 4 - 2 ulp
+    yb = np.float32(4.0 - 2.3e-5)
+    zc = np.nextafter(np.nextafter(four, np.float32(8)), np.float32(8))            # 4 + 2 ulp
+    pos = np.array([[one, one, one, 1.0], [xa, one, one, 2.5], [one, yb, one, 1.0], [one, one, zc, 0.75],
+                    [2.0, 1.5, 1.0, 1.0]], dtype=np.float32)
+    prm = oracle_mod.make_params((16.0,) * 3, 3.0, eps)
+    acc, st = oracle_mod.accel(pos, prm, stats=True)
+    d = pos[1:, :3].astype(np.float64) - pos[0, :3].astype(np.float64)
+    s = (d * d).sum(1)
+    rel = np.abs(s - 9.0) / 9.0
+    assert rel[0] < 2.0 ** -20 and 2.0 ** -17 < rel[1] < 2.0 ** -15 and rel[2] < 2.0 ** -20     # the set-up is what it says
+    assert s[0] < 9.0 and s[1] < 9.0 and s[2] > 9.0
+    f = _independent_factor(s, eps)
+    expect = 2.5 * abs(f[0]) * np.sqrt(s[0]) + 0.75 * abs(f[2]) * np.sqrt(s[2])
+    assert st["allowance"][0] == pytest.approx(expect, rel=1e-9)
+    assert st["allowance"][0] > 0
+    assert st["n_in"][0] == 3                                    # A, B, D inside; C outside
+    # seen from the other side: A's and C's allowance is their pair with the target, B and D have none
+    assert st["allowance"][1] == pytest.approx(1.0 * abs(f[0]) * np.sqrt(s[0]), rel=1e-9)
+    assert st["allowance"][3] == pytest.approx(1.0 * abs(f[2]) * np.sqrt(s[2]), rel=1e-9)
+    assert st["allowance"][2] == 0.0 and st["allowance"][4] == 0.0
+    # a band of 2^-8 (or any band that reaches B) would add B's term: the allowance must be smaller than that sum
+    assert st["allowance"][0] < expect + 0.5 * abs(f[1]) * np.sqrt(s[1])
+
+
+def test_r9_allowance_zero_without_near_cutoff_pairs(oracle_mod):
+    """P5: only the pairs at EXACTLY rc (rows 0-3, 0-4 ... the survey's 'pairs at exactly rc') are inside the band;
+    every other row has allowance exactly 0.  Config-1-like uniform particles: a handful of non-zero entries."""
+    rows = golden_lines("p5_eight_particles.txt")
+    pos = np.array([[float(t) for t in r[:4]] for r in rows], dtype=np.float32)
+    prm = oracle_mod.make_params(BOX16, 3.0, 0.1)
+    acc, st = oracle_mod.accel(pos, prm, stats=True)
+    x = pos[:, :3].astype(np.float64)
+    dd = x[None] - x[:, None]
+    dd -= 16.0 * np.round(dd / 16.0)
+    s = (dd * dd).sum(-1)
+    near = (np.abs(s - 9.0) <= 9.0 * 2.0 ** -18) & ~np.eye(len(pos), dtype=bool)
+    assert near.any()                                             # the example has pairs at exactly rc
+    f = _independent_factor(s, np.float32(0.1))
+    expect = (np.where(near, np.abs(f) * np.sqrt(s), 0.0) * pos[:, 3].astype(np.float64)[None, :]).sum(1)
+    assert np.allclose(st["allowance"], expect, rtol=1e-9, atol=0)
+    assert np.all(st["allowance"][~near.any(1)] == 0.0)
+    rng = np.random.default_rng(4)
+    p = np.ones((4000, 4), dtype=np.float32)
+    p[:, :3] = rng.random((4000, 3)) * 16
+    _, st = oracle_mod.accel(p, oracle_mod.make_params(BOX16, 3.0, 0.1), stats=True)
+    # expected number of ordered pairs in a shell of relative half-width 2^-18 in s: N * rho * 4 pi r^2 dr, dr = rc 2^-18 / 2 ... x2 sides
+    frac = np.count_nonzero(st["allowance"]) / 4000.0
+    expect_frac = (4000 / 16.0 ** 3) * 4 * np.pi * 9 * (2 * 3.0 * 2.0 ** -19)
+    assert frac <= 10 * expect_frac + 2.5e-3                      # ~4e-4: at most a few particles (a 2^-8 band would flag ~40 %)
+
+
+def test_r18_error_norms_hand_computed(oracle_mod):
+    """R18 metric on vectors whose norms are obvious: per particle |da| / max(|a_ref|, 1e-4 rms|a_ref|) after the
+    allowance is subtracted (never below 0); global sqrt(sum |da|^2 / sum |a_ref|^2)."""
+    ref = np.array([[3.0, 4.0, 0.0], [0.0, 0.0, 0.0], [0.0, 0.0, 2.0], [1.0, 2.0, 2.0]])
+    got = np.array([[3.0, 4.0, 0.5], [0.0, 3e-4, 4e-4], [0.0, 0.0, 2.0], [1.0, 2.0, 2.0 + 0.3]])
+    per, glob = oracle_mod.error_norms(got, ref)
+    rms = math.sqrt((25.0 + 0.0 + 4.0 + 9.0) / 4.0)
+    assert per[0] == pytest.approx(0.5 / 5.0, rel=1e-15)
+    assert per[1] == pytest.approx(5e-4 / (1e-4 * rms), rel=1e-12)        # the floor case a_ref = 0
+    assert per[2] == 0.0
+    assert per[3] == pytest.approx(0.3 / 3.0, rel=1e-12)
+    assert glob == pytest.approx(math.sqrt((0.25 + 25e-8 + 0.09) / 38.0), rel=1e-12)
+    # allowance: subtracted from the per-particle numerator, clamped at 0, NOT applied to the global norm
+    per2, glob2 = oracle_mod.error_norms(got, ref, allowance=np.array([0.2, 1.0, 0.0, 0.3 + 1e-3]))
+    assert per2[0] == pytest.approx(0.3 / 5.0, rel=1e-12)
+    assert per2[1] == 0.0 and per2[3] == 0.0
+    assert glob2 == glob
+    # float32 [n,4] input (the GPU's layout): .w is ignored
+    got4 = np.zeros((4, 4), dtype=np.float32)
+    got4[:, :3] = got
+    got4[:, 3] = 7.0
+    per3, glob3 = oracle_mod.error_norms(got4, ref)
+    assert np.allclose(per3, per, rtol=1e-6) and glob3 == pytest.approx(glob, rel=1e-6)
+    # all-zero reference (perfect lattice): the global norm falls back to the absolute one
+    per4, glob4 = oracle_mod.error_norms(np.full((2, 3), 1e-7), np.zeros((2, 3)))
+    assert glob4 == pytest.approx(math.sqrt(6e-14), rel=1e-12) and np.all(np.isfinite(per4))
+
+
+# --------------------------------------------------------- sub-cycle (PAPER.md:73; reading R20) --
+
+def test_subcycle_two_particles_by_hand(oracle_mod):
+    """One sub-step of two equal masses, worked by hand from P1's printed accelerations: they start 0.5 apart moving
+    apart with relative speed 2, so the half stream (dt/2 = 0.25) takes them to EXACTLY 1.0 apart, the kick uses the
+    printed a(d = 1.0, eps), and the second half stream uses the kicked velocity.  Pins the order stream-accel-kick-
+    stream, the half step, the signs, and that the kick factor is kdt (not dt)."""
+    rows = {(float(r[0]), float(r[1])): float(r[3]) for r in golden_lines("p1_two_particle.txt")}
+    for eps in (0.1, 0.05, 0.02):
+        a1 = rows[(1.0, eps)]                              # a = d f at d = 1
+        pos = np.array([[5.0, 7.0, 9.0, 1.0], [5.5, 7.0, 9.0, 1.0]], dtype=np.float32)
+        vel = np.array([[-1.0, 0.25, 0.0, 0.0], [1.0, 0.25, 0.0, 0.0]], dtype=np.float32)
+        dt, kdt = 0.5, 0.125
+        x, v, a = oracle_mod.subcycle(pos, vel, oracle_mod.make_params((32.0,) * 3, 3.0, eps), dt, kdt, 1)
+        # by hand, in fp64 (all inputs are dyadic, so the only fp32 roundings are those of a, v' and x')
+        v0x, v1x = -1.0 + kdt * a1, 1.0 - kdt * a1          # particle 0 is pulled towards +x, particle 1 towards -x
+        assert a[0, 0] == pytest.approx(a1, rel=3e-7) and a[1, 0] == pytest.approx(-a1, rel=3e-7)
+        assert v[0, 0] == pytest.approx(v0x, rel=3e-7) and v[1, 0] == pytest.approx(v1x, rel=3e-7)
+        assert x[0, 0] == pytest.approx(4.75 + 0.25 * v0x, rel=3e-7)
+        assert x[1, 0] == pytest.approx(5.75 + 0.25 * v1x, rel=3e-7)
+        assert v[0, 1] == 0.25 and x[0, 1] == 7.0 + 0.5 * 0.25 and x[0, 2] == 9.0    # free drift across the pair axis
+        assert np.all(a[:, 3] == 0.0) and np.array_equal(x[:, 3], pos[:, 3])
+
+
+def test_subcycle_is_the_composition_and_conserves_momentum(oracle_mod):
+    pos, box = workloads.scaled_clustered(1200, (4, 4, 4), seed=6, frac_halo=0.5, n_halo=3, a_range=(0.5, 1.5))
+    rng = np.random.default_rng(6)
+    vel = np.zeros_like(pos)
+    vel[:, :3] = rng.normal(0, 0.3, (pos.shape[0], 3))
+    prm = oracle_mod.make_params(box, 3.0, 0.1)
+    dt = 0.02
+    # nsub = 1 is stream(dt/2), accel, kick, stream(dt/2), composed by hand: bit-exact
+    x1 = oracle_mod.stream(pos, vel, np.float32(0.5) * np.float32(dt), box)
+    a64 = oracle_mod.accel(x1, prm)
+    a32 = np.zeros_like(pos)
+    a32[:, :3] = a64.astype(np.float32)
+    v1 = oracle_mod.kick(vel, a32, dt)
+    x2 = oracle_mod.stream(x1, v1, np.float32(0.5) * np.float32(dt), box)
+    x, v, a = oracle_mod.subcycle(pos, vel, prm, dt, dt, 1)
+    assert np.array_equal(x, x2) and np.array_equal(v, v1) and np.array_equal(a, a32)
+    # three sub-steps in one call == three calls of one
+    xa, va = pos, vel
+    for _ in range(3):
+        xa, va, aa = oracle_mod.subcycle(xa, va, prm, dt, dt, 1)
+    xb, vb, ab = oracle_mod.subcycle(pos, vel, prm, dt, dt, 3)
+    assert np.array_equal(xa, xb) and np.array_equal(va, vb) and np.array_equal(aa, ab)
+    # equal masses: total momentum is conserved up to the fp32 rounding of the kicks
+    p0, p3 = vel[:, :3].astype(np.float64).sum(0), vb[:, :3].astype(np.float64).sum(0)
+    kick_scale = 3 * dt * np.abs(ab[:, :3].astype(np.float64)).sum()
+    assert np.max(np.abs(p3 - p0)) <= 1e-6 * kick_scale
+    assert np.max(np.abs(vb[:, :3] - vel[:, :3])) > 1e-3          # and the particles were really kicked
+
+
+def test_subcycle_time_reversal(oracle_mod):
+    """The symmetric split is time reversible: nsub steps forward, flip v, nsub steps forward again returns to the
+    start up to the fp32 rounding of x and v.  (A missing half factor, or kick and stream in another order such as
+    kick-stream-stream, would leave an O(dt^2 a) error, four orders of magnitude above this bound.)"""
+    pos, box = workloads.scaled_clustered(600, (3, 3, 4), seed=8, frac_halo=0.4, n_halo=2, a_range=(0.8, 1.5))
+    rng = np.random.default_rng(1)
+    vel = np.zeros_like(pos)
+    vel[:, :3] = rng.normal(0, 0.2, (pos.shape[0], 3))
+    prm = oracle_mod.make_params(box, 3.0, 0.1)
+    dt, nsub = 0.01, 4
+    x, v, _ = oracle_mod.subcycle(pos, vel, prm, dt, dt, nsub)
+    v[:, :3] *= -1
+    xr, vr, _ = oracle_mod.subcycle(x, v, prm, dt, dt, nsub)
+    d = xr[:, :3].astype(np.float64) - pos[:, :3]
+    d -= np.asarray(box) * np.round(d / np.asarray(box))
+    moved = x[:, :3].astype(np.float64) - pos[:, :3]
+    moved -= np.asarray(box) * np.round(moved / np.asarray(box))
+    assert np.max(np.abs(moved)) > 1e-3
+    assert np.max(np.abs(d)) < 2e-5 and np.max(np.abs(vr[:, :3] + vel[:, :3])) < 2e-5
