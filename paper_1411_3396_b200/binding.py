@@ -247,10 +247,11 @@ class Solver:
         nh, n = int(hs.shape[0]) - 1, int(pos_mass.shape[0])
         nbytes = C.c_size_t(0)
         self._check(self.lib.srpp_mbp_workspace_bytes(n, nh, C.byref(nbytes)), "srpp_mbp_workspace_bytes")
-        ws = torch.empty(max(int(nbytes.value), 256), dtype=torch.uint8, device=self.device)
-        idx = torch.empty(max(nh, 1), dtype=torch.int64, device=self.device)[:nh]
-        pmin = torch.empty(max(nh, 1), dtype=torch.float32, device=self.device)[:nh]
-        phi = torch.zeros(max(n, 1), dtype=torch.float32, device=self.device)[:n] if want_phi else None
+        with torch.cuda.stream(self.stream):           # allocated (and zeroed) on the stream the kernels run on
+            ws = torch.empty(max(int(nbytes.value), 256), dtype=torch.uint8, device=self.device)
+            idx = torch.empty(max(nh, 1), dtype=torch.int64, device=self.device)[:nh]
+            pmin = torch.empty(max(nh, 1), dtype=torch.float32, device=self.device)[:nh]
+            phi = torch.zeros(max(n, 1), dtype=torch.float32, device=self.device)[:n] if want_phi else None
         self._check(self.lib.srpp_mbp(self._ctx, pos_mass.data_ptr(), n, hs.ctypes.data_as(C.POINTER(C.c_int64)), nh,
                                       phi.data_ptr() if want_phi else None, idx.data_ptr(), pmin.data_ptr(),
                                       ws.data_ptr(), int(nbytes.value)), "srpp_mbp")

@@ -53,7 +53,12 @@ static int32_t validate(const srpp_params* p) {
   if (!p) return SRPP_ERR_INVALID_ARG;
   for (int a = 0; a < 3; ++a)
     if (!(p->box[a] > 0.f) || !isfinite(p->box[a])) return SRPP_ERR_INVALID_ARG;
+  // the force kernel stages coordinates relative to INTEGER reference points (exact periodic shifts in fp32): the box
+  // and the cutoff must stay inside fp32's exact-integer range
+  for (int a = 0; a < 3; ++a)
+    if (p->box[a] > 16777216.f) return SRPP_ERR_GEOMETRY;
   if (!(p->rcut > 0.f) || !isfinite(p->rcut) || !(p->eps > 0.f) || !isfinite(p->eps)) return SRPP_ERR_INVALID_ARG;
+  if (p->rcut > 16777216.f) return SRPP_ERR_GEOMETRY;
   for (int k = 0; k < 6; ++k)
     if (!isfinite(p->poly[k])) return SRPP_ERR_INVALID_ARG;
   int64_t ncells = 1;
@@ -64,6 +69,18 @@ static int32_t validate(const srpp_params* p) {
     if (ncells > (1 << 24)) return SRPP_ERR_GEOMETRY;
   }
   return SRPP_OK;
+}
+
+// float4 arrays must be 16-byte aligned (vector loads/stores, cp.async 16): a misaligned pointer would raise a sticky
+// misaligned-address fault instead of a status code
+static inline bool misaligned16(const void* p) { return ((uintptr_t)p & 15u) != 0; }
+
+// Every compute call runs on the device that was current at srpp_create (kernel attributes and occupancy are cached
+// per context): a different current device is a state error, not a silent launch on the wrong GPU.
+static int32_t check_device(const srpp_ctx* c) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SRPP_ERR_CUDA;
+  return dev == c->device ? SRPP_OK : SRPP_ERR_STATE;
 }
 
 static int32_t cuda_fail(srpp_ctx* c, cudaError_t e) {
@@ -138,6 +155,12 @@ int32_t srpp_create(srpp_ctx** out, const srpp_params* params, void* workspace, 
   c->fc.eps2 = (float)e2;
   const double e2f = (double)c->fc.eps2;
   c->fc.rc2e = (float)((double)params->rcut * (double)params->rcut + e2f);
+  {  // padding coordinate of empty target / source slots: farther than rc from every real relative coordinate
+     // (targets lie within [0, cell_w + 1] of their reference point, sources within [-cell_w - 1, 2 cell_w + 2])
+    float wmax = 0.f;
+    for (int a = 0; a < 3; ++a) wmax = fmaxf(wmax, params->box[a] / (float)params->ncell[a]);
+    c->fc.pad = 8.f * wmax + 4.f * params->rcut + 16.f;
+  }
   double q[6];
   for (int k = 0; k < 6; ++k) {
     double acc = 0.0, binom = 1.0, powr = 1.0;   // sum_{j>=k} c_j C(j,k) (-e2f)^(j-k)
@@ -224,51 +247,56 @@ int32_t srpp_set_boundary(srpp_ctx* c, const int32_t* periodic_host, const float
                           const float* active_hi_host) {
   if (!c) return SRPP_ERR_INVALID_ARG;
   Geometry& g = c->geo;
+  int32_t per[3], clo[3], chi[3];       // validated into temporaries: the boundary is unchanged on error
   for (int a = 0; a < 3; ++a) {
-    const int32_t per = periodic_host ? (periodic_host[a] != 0) : 1;
+    per[a] = periodic_host ? (periodic_host[a] != 0) : 1;
     float lo = active_lo_host ? active_lo_host[a] : 0.f, hi = active_hi_host ? active_hi_host[a] : c->params.box[a];
     if (!(lo <= hi) || !isfinite(lo) || !isfinite(hi)) return SRPP_ERR_INVALID_ARG;
     lo = fmaxf(lo, 0.f);
     hi = fminf(hi, c->params.box[a]);
     // cells [clo, chi) that can hold a particle with lo <= x < hi: the fp32 cell function of A1 (R10) is monotonic
     // in x, so the cells of lo and of the largest float below hi bound the range
-    int32_t clo = (int32_t)floorf(lo * g.inv_cell[a]);
-    int32_t chi = (int32_t)floorf(nextafterf(hi, -INFINITY) * g.inv_cell[a]) + 1;
-    if (clo > g.ncell[a] - 1) clo = g.ncell[a] - 1;
-    if (clo < 0) clo = 0;
-    if (chi > g.ncell[a]) chi = g.ncell[a];
-    if (hi <= lo) chi = clo;
-    g.periodic[a] = per;
-    g.act_lo[a] = clo;
-    g.act_hi[a] = chi;
+    clo[a] = (int32_t)floorf(lo * g.inv_cell[a]);
+    chi[a] = (int32_t)floorf(nextafterf(hi, -INFINITY) * g.inv_cell[a]) + 1;
+    if (clo[a] > g.ncell[a] - 1) clo[a] = g.ncell[a] - 1;
+    if (clo[a] < 0) clo[a] = 0;
+    if (chi[a] > g.ncell[a]) chi[a] = g.ncell[a];
+    if (hi <= lo) chi[a] = clo[a];
+  }
+  for (int a = 0; a < 3; ++a) {
+    g.periodic[a] = per[a];
+    g.act_lo[a] = clo[a];
+    g.act_hi[a] = chi[a];
   }
   return SRPP_OK;
 }
 
 int32_t srpp_mbp_workspace_bytes(int64_t n, int64_t nhalo, size_t* bytes_host) {
-  if (!bytes_host || n < 0 || n >= ((int64_t)1 << 31) || nhalo < 0 || nhalo >= ((int64_t)1 << 31)) return SRPP_ERR_INVALID_ARG;
-  size_t a, b, d;
-  *bytes_host = mbp_workspace_layout(n, nhalo, &a, &b, &d);
+  if (!bytes_host || n < 0 || n >= ((int64_t)1 << 31) || nhalo < 0 || nhalo > ((int64_t)1 << 24)) return SRPP_ERR_INVALID_ARG;
+  size_t a, b, d, t;
+  *bytes_host = mbp_workspace_layout(n, nhalo, &a, &b, &d, &t);
   return SRPP_OK;
 }
 
 int32_t srpp_mbp(srpp_ctx* c, const float* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
                  float* phi, int64_t* mbp_index, float* mbp_phi, void* workspace, size_t workspace_bytes) {
-  if (!c || n < 0 || n >= ((int64_t)1 << 31) || nhalo < 0 || nhalo >= ((int64_t)1 << 31) || !halo_start_host ||
-      (n > 0 && !pos_mass) || (nhalo > 0 && !mbp_index) || !workspace)
+  if (!c || n < 0 || n >= ((int64_t)1 << 31) || nhalo < 0 || nhalo > ((int64_t)1 << 24) || !halo_start_host ||
+      (n > 0 && !pos_mass) || (nhalo > 0 && !mbp_index) || !workspace || misaligned16(pos_mass))
     return SRPP_ERR_INVALID_ARG;
+  if (const int32_t d = check_device(c)) return d;
   if (halo_start_host[0] < 0 || halo_start_host[nhalo] > n) return SRPP_ERR_INVALID_ARG;
   for (int64_t h = 0; h < nhalo; ++h)
     if (halo_start_host[h + 1] < halo_start_host[h]) return SRPP_ERR_INVALID_ARG;
-  size_t a, b, d;
-  if (((uintptr_t)workspace & 255u) != 0 || workspace_bytes < mbp_workspace_layout(n, nhalo, &a, &b, &d)) return SRPP_ERR_WORKSPACE;
+  size_t a, b, d, t;
+  if (((uintptr_t)workspace & 255u) != 0 || workspace_bytes < mbp_workspace_layout(n, nhalo, &a, &b, &d, &t)) return SRPP_ERR_WORKSPACE;
   const cudaError_t e = launch_mbp(c, (const float4*)pos_mass, n, halo_start_host, nhalo, phi, (long long*)mbp_index,
                                    mbp_phi, (char*)workspace);
   return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
 }
 
 int32_t srpp_build_mesh(srpp_ctx* c, const float* pos_mass, int64_t n) {
-  if (!c || n < 0 || n >= ((int64_t)1 << 31) || (n > 0 && !pos_mass)) return SRPP_ERR_INVALID_ARG;
+  if (!c || n < 0 || n >= ((int64_t)1 << 31) || (n > 0 && !pos_mass) || misaligned16(pos_mass)) return SRPP_ERR_INVALID_ARG;
+  if (const int32_t d = check_device(c)) return d;
   c->n = -1;
   if (workspace_layout(c->params, n, nullptr) > c->ws_bytes) return SRPP_ERR_WORKSPACE;
   workspace_layout(c->params, n, c);
@@ -299,7 +327,8 @@ int32_t srpp_get_mesh(const srpp_ctx* c, const uint32_t** cell_start, const uint
 int32_t srpp_accel(srpp_ctx* c, float* acc) {
   if (!c) return SRPP_ERR_INVALID_ARG;
   if (c->n < 0) return SRPP_ERR_STATE;
-  if (c->n > 0 && !acc) return SRPP_ERR_INVALID_ARG;
+  if ((c->n > 0 && !acc) || misaligned16(acc)) return SRPP_ERR_INVALID_ARG;
+  if (const int32_t d = check_device(c)) return d;
   const cudaError_t e = launch_accel(c, (float4*)acc);
   return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
 }
@@ -320,20 +349,22 @@ int32_t srpp_get_stats(srpp_ctx* c, srpp_stats* s) {
 }
 
 int32_t srpp_kick(srpp_ctx* c, float* vel, const float* acc, float kdt, int64_t n) {
-  if (!c || n < 0 || (n > 0 && (!vel || !acc)) || !isfinite(kdt)) return SRPP_ERR_INVALID_ARG;
+  if (!c || n < 0 || (n > 0 && (!vel || !acc)) || !isfinite(kdt) || misaligned16(vel) || misaligned16(acc)) return SRPP_ERR_INVALID_ARG;
+  if (const int32_t d = check_device(c)) return d;
   const cudaError_t e = launch_kick(c, (float4*)vel, (const float4*)acc, kdt, n);
   return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
 }
 
 int32_t srpp_stream(srpp_ctx* c, float* pos_mass, const float* vel, float dt, int64_t n) {
-  if (!c || n < 0 || (n > 0 && (!pos_mass || !vel)) || !isfinite(dt)) return SRPP_ERR_INVALID_ARG;
+  if (!c || n < 0 || (n > 0 && (!pos_mass || !vel)) || !isfinite(dt) || misaligned16(pos_mass) || misaligned16(vel)) return SRPP_ERR_INVALID_ARG;
+  if (const int32_t d = check_device(c)) return d;
   const cudaError_t e = launch_stream(c, (float4*)pos_mass, (const float4*)vel, dt, n);
   return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
 }
 
 int32_t srpp_step_host(srpp_ctx* c, const float* pos_mass_host, float* vel_host, float* acc_host, float kdt,
                        int64_t n, void* device_scratch, size_t device_scratch_bytes) {
-  if (!c || n < 0 || (n > 0 && (!pos_mass_host || !acc_host || !device_scratch))) return SRPP_ERR_INVALID_ARG;
+  if (!c || n < 0 || n >= ((int64_t)1 << 31) || (n > 0 && (!pos_mass_host || !acc_host || !device_scratch))) return SRPP_ERR_INVALID_ARG;
   const size_t bytes = 16 * (size_t)n;
   if (device_scratch_bytes < 3 * bytes || ((uintptr_t)device_scratch & 15u)) return SRPP_ERR_WORKSPACE;
   float* d_pos = (float*)device_scratch;

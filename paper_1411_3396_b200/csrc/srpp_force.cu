@@ -8,10 +8,11 @@
 //     (exclusive prefix over cells); autonomous WARPS pull item indices from one atomic counter, so a
 //     cell holding 600 k particles becomes ~10^6 small items spread over the whole chip -- the on-chip
 //     analogue of the paper's block splitting for load balance.
-//   * Targets live in registers as PACKED PAIRS (float2 = two targets), sources are broadcast from a
-//     warp-private shared-memory tile stored duplicated (x,x,y,y | z,z | m,m) so that every arithmetic
-//     instruction of the pair loop is a Blackwell packed-fp32 op (FFMA2/FADD2/FMUL2): 16 packed FMA-pipe
-//     instructions per two pair interactions, leaving issue slots for MUFU.RSQ and the cutoff select.
+//   * Targets live in registers as PACKED PAIRS (float2 = two targets); sources are staged by the warp into a
+//     private shared-memory tile of float4 (x, y, z, m), read with one LDS.128 per source and fed to the packed
+//     instructions as broadcast operands, so that every arithmetic instruction of the pair loop is a Blackwell
+//     packed-fp32 op (FFMA2/FADD2/FMUL2): 16 packed FMA-pipe instructions per two pair interactions, leaving
+//     issue slots for MUFU.RSQ and the cutoff select.
 //   * Periodic images are applied when a source segment is staged (a per-segment shift), never per pair.
 //     Staged coordinates are relative to integer reference points, so the wrap is exact in fp32.
 //   * u = s + eps^2 comes straight out of the FMA chain (seeded with eps^2); the grid-force polynomial
@@ -213,7 +214,7 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
 #pragma unroll
   for (int t = 0; t < TP; ++t) {
     const uint32_t k0 = tgt_begin + t * (64 / S) + (lane & (32 / S - 1)), k1 = k0 + 32 / S;
-    float4 a = make_float4(-1.0e3f, -1.0e3f, -1.0e3f, 0.f), b = a;
+    float4 a = make_float4(-fc.pad, -fc.pad, -fc.pad, 0.f), b = a;   // empty target slot: beyond rc of every source
     if (k0 < tgt_end) { a = __ldg(&sorted[k0]); a.x -= ref_t[0]; a.y -= ref_t[1]; a.z -= ref_t[2]; }
     if (k1 < tgt_end) { b = __ldg(&sorted[k1]); b.x -= ref_t[0]; b.y -= ref_t[1]; b.z -= ref_t[2]; }
     ntx[t] = make_float2(-a.x, -b.x);
@@ -238,7 +239,7 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
 #pragma unroll
     for (int j = 0; j < kSrcTile / 32; ++j) {
       const uint32_t p = tile + j * 32 + lane;
-      float4 sv = make_float4(1.0e3f, 1.0e3f, 1.0e3f, 0.f);
+      float4 sv = make_float4(fc.pad, fc.pad, fc.pad, 0.f);   // empty source slot: cut off for every target (scale-independent)
       if (p < p1) {
         while (p >= ws.seg_start[seg + 1]) ++seg;
         const float4 v = __ldg(&sorted[ws.seg_base[seg] + (p - ws.seg_start[seg])]);
@@ -343,12 +344,13 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
       lo = nlo;
     }
     const int c = lo;
-    const uint32_t local = (uint32_t)(idx - __ldg(&item_prefix[c]));
+    const unsigned long long local = idx - __ldg(&item_prefix[c]);   // 64-bit: one cell can hold > 2^32 items
     const uint32_t cs0 = __ldg(&cell_start[c]), cs1 = __ldg(&cell_start[c + 1]);
     const uint32_t n_c = cs1 - cs0;
     const uint32_t tpi = targets_per_item(n_c, fc.fine_items);
     const uint32_t ntile = (n_c + tpi - 1) / tpi;
-    const uint32_t tile = local % ntile, chunk = local / ntile;   // chunk-major: neighbours share sources
+    const uint32_t tile = (uint32_t)(local % ntile);              // chunk-major: neighbours share sources
+    const unsigned long long chunk = local / ntile;
     const int cx = c % g.ncell[0], cy = (c / g.ncell[0]) % g.ncell[1], cz = c / (g.ncell[0] * g.ncell[1]);
 
     // ---- segment table of this cell's source stream (lanes 0..17), prefix by warp scan
@@ -380,7 +382,7 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
     if (lane == 0) ws.seg_start[kMaxSeg] = S;
     __syncwarp();
 
-    const uint32_t p0 = chunk * kSrcChunk, p1 = min(S, p0 + kSrcChunk);
+    const uint32_t p0 = (uint32_t)min(chunk * (unsigned long long)kSrcChunk, (unsigned long long)S), p1 = min(S, p0 + kSrcChunk);
     const uint32_t tb = cs0 + tile * tpi, te = min(cs1, tb + tpi);
     if (n_c <= 16u || (fc.fine_items && n_c <= kSplitMaxCell))
       process_item<1, kUniformMass, kSplit>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
@@ -460,6 +462,15 @@ int query_force_occupancy() {
   return m < 1 ? 1 : m;
 }
 
+cudaError_t launch_scan_u64(cudaStream_t st, unsigned long long* data, int n, unsigned long long* tmp,
+                            unsigned long long* total_out, unsigned long long* total_out2) {
+  const int nb = (n + kScanBlock - 1) / kScanBlock;     // <= 4096 blocks (n <= 2^24): one top-level block scans them
+  k_scan_reduce<<<nb, kScanThreads, 0, st>>>(data, n, tmp);
+  k_scan_top<<<1, kScanThreads, 0, st>>>(tmp, nb, total_out, total_out2);
+  k_scan_apply<<<nb, kScanThreads, 0, st>>>(data, n, tmp);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
   cudaStream_t st = c->stream;
   const int64_t n = c->n;
@@ -472,10 +483,7 @@ cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
   if ((e = cudaMemsetAsync(c->acc64, 0, sizeof(double) * 3 * (size_t)n, st)) != cudaSuccess) return e;
   c->fc.fine_items = n < (int64_t)c->num_sms * c->force_blocks_per_sm * kForceWarps * 64 ? 1 : 0;   // < 64 particles per resident warp
   k_plan_items<<<(ncells + 255) / 256, 256, 0, st>>>(c->cell_start, c->geo, c->fc.fine_items, c->item_prefix, c->flags);
-  const int nb = (ncells + kScanBlock - 1) / kScanBlock;
-  k_scan_reduce<<<nb, kScanThreads, 0, st>>>(c->item_prefix, ncells, c->scan_tmp);
-  k_scan_top<<<1, kScanThreads, 0, st>>>(c->scan_tmp, nb, &c->flags->total_items, &c->item_prefix[ncells]);
-  k_scan_apply<<<nb, kScanThreads, 0, st>>>(c->item_prefix, ncells, c->scan_tmp);
+  if ((e = launch_scan_u64(st, c->item_prefix, ncells, c->scan_tmp, &c->flags->total_items, &c->item_prefix[ncells])) != cudaSuccess) return e;
   const int grid = c->num_sms * c->force_blocks_per_sm;
   if (c->timing) cudaEventRecord(c->ev[kEvForce0], st);
   if (c->uniform_mass)

@@ -57,6 +57,7 @@ struct ForceConst {
   float eps2;            // eps^2 rounded to fp32: seeds the s-FMA chain, u = s + eps2
   float rc2e;            // rc^2 + eps2: cutoff test on u
   float nq[6];           // -Q(u) coefficients, Q(u) = P(u - eps2), expanded in fp64
+  float pad;             // coordinate of padded (empty) target / source slots: beyond rc of every real one at any scale
   int32_t fine_items;    // tiny problem: 16-target items so that every resident warp gets work
 };
 
@@ -104,7 +105,7 @@ struct srpp_ctx {
   cudaEvent_t ev[srpp::kNumEvents];
   bool ev_mesh_valid, ev_accel_valid;
   uint64_t launches;         // kernels launched by this context so far (harness evidence)
-  unsigned long long mbp_pairs;  // sum of n_h^2 of the last srpp_mbp call (ordered pairs incl. self, the metric's unit)
+  int mbp_occ;               // resident CTAs per SM of k_mbp_phi (queried once)
 };
 
 namespace srpp {
@@ -119,8 +120,11 @@ cudaError_t launch_accel(srpp_ctx* c, float4* acc);
 cudaError_t launch_kick(srpp_ctx* c, float4* vel, const float4* acc, float kdt, int64_t n);
 cudaError_t launch_stream(srpp_ctx* c, float4* pos_mass, const float4* vel, float dt, int64_t n);
 int query_force_occupancy();
+// in-place exclusive scan of data[0..n) (n <= 2^24); the total goes to *total_out and *total_out2 (device pointers)
+cudaError_t launch_scan_u64(cudaStream_t st, unsigned long long* data, int n, unsigned long long* tmp,
+                            unsigned long long* total_out, unsigned long long* total_out2);
 // srpp_mbp.cu
-size_t mbp_workspace_layout(int64_t n, int64_t nhalo, size_t* o_phi, size_t* o_prefix, size_t* o_start);
+size_t mbp_workspace_layout(int64_t n, int64_t nhalo, size_t* o_phi, size_t* o_prefix, size_t* o_start, size_t* o_tmp);
 cudaError_t launch_mbp(srpp_ctx* c, const float4* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
                        float* phi_out, long long* mbp_index, float* mbp_phi, char* ws);
 // srpp_probe.cu

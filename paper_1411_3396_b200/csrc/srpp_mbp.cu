@@ -5,7 +5,7 @@
 // The paper builds this from Thrust scan/transform/reduce on Titan's K20X; here it is the second O(n^2) workload on
 // the pair-tile machinery of the force kernel:
 //   * work item = (halo h, tile of <= 128 members as targets, chunk of <= 1024 members as sources); all items of all
-//     halos form one index space (exclusive prefix over halos, computed on the host from halo_start) and autonomous
+//     halos form one index space (exclusive prefix over halos, computed on the device from halo_start) and autonomous
 //     warps pull items from one atomic counter, so a 4-million-particle halo spreads over the whole chip while 10^5
 //     small halos fill it just as well (the paper's load imbalance across halos);
 //   * targets in registers as packed pairs, sources staged per warp as float4 (x, y, z, m) relative to the halo's first
@@ -14,7 +14,6 @@
 //   * <= 1024 fp32 terms per item, folded into fp64 with red.global.add.f64; a second kernel negates, removes the self
 //     term and reduces (phi, index) per halo.
 #include <algorithm>
-#include <vector>
 
 #include "srpp_internal.cuh"
 
@@ -156,52 +155,54 @@ __global__ void __launch_bounds__(256) k_mbp_reduce(const float4* __restrict__ p
   }
 }
 
-size_t mbp_workspace_layout(int64_t n, int64_t nhalo, size_t* o_phi, size_t* o_prefix, size_t* o_start) {
+// items per halo (target tiles x source chunks), before the exclusive scan
+__global__ void __launch_bounds__(256) k_mbp_items(const long long* __restrict__ halo_start, int nhalo,
+                                                    unsigned long long* __restrict__ items) {
+  const int h = blockIdx.x * blockDim.x + threadIdx.x;
+  if (h >= nhalo) return;
+  const unsigned long long nh = (unsigned long long)(__ldg(&halo_start[h + 1]) - __ldg(&halo_start[h]));
+  items[h] = ((nh + kMbpTargets - 1) / kMbpTargets) * ((nh + kMbpChunk - 1) / kMbpChunk);
+}
+
+size_t mbp_workspace_layout(int64_t n, int64_t nhalo, size_t* o_phi, size_t* o_prefix, size_t* o_start, size_t* o_tmp) {
   auto up = [](size_t x) { return (x + 255) / 256 * 256; };
   size_t off = 256;                                   // counter block
   *o_phi = off; off = up(off + 8 * (size_t)(n > 0 ? n : 1));
   *o_prefix = off; off = up(off + 8 * (size_t)(nhalo + 1));
   *o_start = off; off = up(off + 8 * (size_t)(nhalo + 1));
+  *o_tmp = off; off = up(off + 8 * ((size_t)nhalo / 4096 + 2));
   return off;
 }
 
+// The halo table is read from host memory during the call (one pageable->device copy: the runtime stages it before
+// returning, so the caller's buffer is free on return); the item prefix is computed on the device.  No stream sync.
 cudaError_t launch_mbp(srpp_ctx* c, const float4* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
                        float* phi_out, long long* mbp_index, float* mbp_phi, char* ws) {
   cudaStream_t st = c->stream;
-  size_t o_phi, o_prefix, o_start;
-  mbp_workspace_layout(n, nhalo, &o_phi, &o_prefix, &o_start);
+  size_t o_phi, o_prefix, o_start, o_tmp;
+  mbp_workspace_layout(n, nhalo, &o_phi, &o_prefix, &o_start, &o_tmp);
   unsigned long long* counter = (unsigned long long*)ws;
   double* phi64 = (double*)(ws + o_phi);
   unsigned long long* prefix = (unsigned long long*)(ws + o_prefix);
   long long* hs = (long long*)(ws + o_start);
-  std::vector<unsigned long long> pre((size_t)nhalo + 1);
-  pre[0] = 0;
-  for (int64_t h = 0; h < nhalo; ++h) {
-    const unsigned long long nh = (unsigned long long)(halo_start_host[h + 1] - halo_start_host[h]);
-    pre[h + 1] = pre[h] + ((nh + kMbpTargets - 1) / kMbpTargets) * ((nh + kMbpChunk - 1) / kMbpChunk);
-  }
+  unsigned long long* tmp = (unsigned long long*)(ws + o_tmp);
   cudaError_t e;
   if ((e = cudaMemsetAsync(counter, 0, 256, st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(phi64, 0, 8 * (size_t)(n > 0 ? n : 1), st)) != cudaSuccess) return e;
-  if ((e = cudaMemcpyAsync(prefix, pre.data(), 8 * pre.size(), cudaMemcpyHostToDevice, st)) != cudaSuccess) return e;
   if ((e = cudaMemcpyAsync(hs, halo_start_host, 8 * ((size_t)nhalo + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess) return e;
-  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return e;     // `pre` is a local: the copy must have left it
+  if (nhalo == 0) return cudaSuccess;
+  k_mbp_items<<<(int)((nhalo + 255) / 256), 256, 0, st>>>(hs, (int)nhalo, prefix);
+  if ((e = launch_scan_u64(st, prefix, (int)nhalo, tmp, &prefix[nhalo], counter + 8)) != cudaSuccess) return e;
   const float eps2 = c->fc.eps2;
-  if (pre[nhalo] > 0) {
+  if (!c->mbp_occ) {
     int occ = 1;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mbp_phi, kForceThreads, 0)) != cudaSuccess) return e;
-    k_mbp_phi<<<c->num_sms * std::max(occ, 1), kForceThreads, 0, st>>>(pos_mass, hs, prefix, (int)nhalo, eps2, counter, phi64);
-    c->launches += 1;
+    c->mbp_occ = std::max(occ, 1);
   }
-  if (nhalo == 0) return cudaSuccess;
+  k_mbp_phi<<<c->num_sms * c->mbp_occ, kForceThreads, 0, st>>>(pos_mass, hs, prefix, (int)nhalo, eps2, counter, phi64);
   const int grid = (int)std::min<int64_t>(nhalo, (int64_t)c->num_sms * 8);
   k_mbp_reduce<<<grid, 256, 0, st>>>(pos_mass, hs, (int)nhalo, eps2, phi64, phi_out, mbp_index, mbp_phi);
-  c->launches += 1;
-  c->mbp_pairs = 0;
-  for (int64_t h = 0; h < nhalo; ++h) {
-    const unsigned long long nh = (unsigned long long)(halo_start_host[h + 1] - halo_start_host[h]);
-    c->mbp_pairs += nh * nh;
-  }
+  c->launches += 6;
   return cudaGetLastError();
 }
 

@@ -12,7 +12,6 @@ GOLDEN = os.path.join(ROOT, "tests", "golden")
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
-    config.addinivalue_line("markers", "full: full-size configs 3-5 (minutes; enabled with SRPP_FULL=1)")
 
 
 def golden_lines(name):

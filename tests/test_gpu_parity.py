@@ -174,7 +174,10 @@ def test_accel_two_particles_and_cutoff(oracle_mod, gpu):
         # absolute bound of the fp32 evaluation of r^3 - Q(u) (two ~0.04 terms cancelling): |df| <= 2e-7
         # (DESIGN.md "fp32 error budget").  In a real neighbourhood this is far below 1e-3 of |a|.
         dd = float(pos[1, 0]) - float(pos[0, 0])
-        assert np.all(np.abs(a[:, :3] - ref) <= np.maximum(1e-3 * np.abs(ref), 2e-7 * dd))
+        err = np.abs(a[:, :3] - ref)
+        print("isolated pair d=%g eps=%g: |da| max %.3e = %.3e relative, %.3e of the absolute bound 2e-7 d"
+              % (d, eps, err.max(), err.max() / max(np.abs(ref).max(), 1e-300), err.max() / (2e-7 * dd)))
+        assert np.all(err <= np.maximum(1e-3 * np.abs(ref), 2e-7 * dd))
         assert np.array_equal(a[0, :3], -a[1, :3])          # same arithmetic on both sides, m = 1
     for d in (3.0, 3.5, 6.0):    # at and beyond the cutoff: exactly zero (R5)
         pos = np.array([[5, 7, 9, 1], [5 + d, 7, 9, 1]], dtype=np.float32)
@@ -257,6 +260,30 @@ def test_accel_uniform_mass_scale_and_custom_poly(oracle_mod, gpu):
     a, sol = _gpu_accel(gpu, pos, box, (5, 5, 5), 0.07, poly=poly)
     assert sol.get_stats()["uniform_mass"] == 1
     _check_accel(oracle_mod, a, pos, box, 0.07, poly=poly, label="custom poly")
+
+
+def test_accel_large_cells_uniform_mass(oracle_mod, gpu):
+    """Padding must not depend on the length scale: a box of 3 x 1200-unit cells with rc = 3 and equal masses (the
+    path that never multiplies by the source mass); cells hold ragged counts so padded slots exist everywhere."""
+    rng = np.random.default_rng(9)
+    box, ncell = (3600.0, 3000.0, 4500.0), (3, 3, 3)
+    n = 6000
+    centres = rng.random((60, 3)) * np.asarray(box)
+    pos = np.ones((n, 4), dtype=np.float32)
+    pos[:, :3] = np.mod(centres[rng.integers(0, 60, n)] + rng.normal(0, 1.5, (n, 3)), np.asarray(box)).astype(np.float32)
+    for big_rc in (False, True):
+        rc = 700.0 if big_rc else 3.0
+        poly = np.zeros(6, dtype=np.float32) if big_rc else None      # the default fit is only meaningful for rc = 3
+        torch, binding = gpu
+        sol = binding.Solver(box, ncell, rc, 0.05, poly=poly, n_max=n)
+        d = torch.from_numpy(pos).cuda()
+        sol.build_mesh(d)
+        a = sol.accel().cpu().numpy()
+        assert sol.get_stats()["uniform_mass"] == 1
+        prm = oracle_mod.make_params(box, rc, 0.05, poly)
+        ref, st = oracle_mod.accel(pos, prm, stats=True)
+        per, glob = oracle_mod.error_norms(a, ref, st["allowance"])
+        assert per.max() <= PER_PARTICLE_TOL and glob <= GLOBAL_L2_TOL, (rc, per.max(), glob)
 
 
 def test_accel_permutation_invariance(oracle_mod, gpu):
@@ -348,17 +375,62 @@ def _sampled_targets(oracle_mod, pos, box, ncell, n_uniform=1024, n_weighted=102
     return np.unique(t), cs, perm, int((cnt * sten).sum())
 
 
-def _full_config(oracle_mod, gpu, cfg, n_uniform, n_weighted):
+def _r17_sequence(oracle_mod, gpu, sol, d_pos, pos, a_gpu, box, ncell, label):
+    """BASELINE.json configs[4] as worded, reading R17: force -> kick(tau) -> stream(tau) -> build mesh again, v0 = 0,
+    tau^2 max|a| = 1.6 (the fastest particle moves half a cell).  Velocities and positions bit-exact against
+    orc_kick / orc_stream fed the GPU's own accelerations, the re-built mesh bit-exact against orc_build_mesh of those
+    positions; returns the fraction of particles that changed cell."""
+    torch, binding = gpu
+    amax = float(np.max(np.abs(a_gpu[:, :3])))
+    tau = float(np.float32(np.sqrt(1.6 / amax)))
+    d_acc = torch.from_numpy(a_gpu).cuda()
+    d_vel = torch.zeros_like(d_pos)
+    sol.kick(d_vel, d_acc, tau)
+    sol.stream_positions(d_pos, d_vel, tau)
+    sol.build_mesh(d_pos)
+    cs, perm, srt = sol.get_mesh()
+    torch.cuda.synchronize()
+    v_ref = oracle_mod.kick(np.zeros_like(pos), a_gpu, tau)
+    assert np.array_equal(d_vel.cpu().numpy().view(np.uint32), v_ref.view(np.uint32))
+    x_ref = oracle_mod.stream(pos, v_ref, tau, box)
+    del v_ref
+    assert np.array_equal(d_pos.cpu().numpy().view(np.uint32), x_ref.view(np.uint32))
+    o_cs, o_perm, o_srt = oracle_mod.build_mesh(x_ref, box, ncell)
+    assert np.array_equal(cs.cpu().numpy().view(np.uint32), o_cs)
+    assert np.array_equal(perm.cpu().numpy().view(np.uint32), o_perm)
+    assert np.array_equal(srt.cpu().numpy().view(np.uint32), o_srt.view(np.uint32))
+    del o_srt, o_perm
+    moved = float(np.mean(oracle_mod.cell_ids(pos, box, ncell) != oracle_mod.cell_ids(x_ref, box, ncell)))
+    print("%s R17: tau = %.4e (max|a| = %.4e), %.3f %% of the particles changed cell" % (label, tau, amax, 100 * moved))
+    return moved
+
+
+def _full_config(oracle_mod, gpu, cfg, n_uniform, n_weighted, r17=False):
+    torch, binding = gpu
     w = workloads.CONFIGS[cfg]
     pos = workloads.generate(cfg)
-    a, sol = _gpu_accel(gpu, pos, w.box, w.ncell, w.eps)
+    sol = _solver(gpu, w.box, w.ncell, w.eps, pos.shape[0])
+    d = torch.from_numpy(pos).cuda()
+    sol.build_mesh(d)
+    acc = sol.accel()
+    torch.cuda.synchronize()
+    a = acc.cpu().numpy()
+    del acc
+    assert np.all(a[:, 3] == 0.0)
     t, o_cs, o_perm, W = _sampled_targets(oracle_mod, pos, w.box, w.ncell, n_uniform, n_weighted)
     st = sol.get_stats()
     assert st["candidate_pairs"] == W
     cs, perm, srt = sol.get_mesh()
     assert np.array_equal(cs.cpu().numpy().view(np.uint32), o_cs)
     assert np.array_equal(perm.cpu().numpy().view(np.uint32), o_perm)
-    _check_accel(oracle_mod, a, pos, w.box, w.eps, targets=t, label="config%d sampled" % cfg)
+    assert np.array_equal(srt.cpu().numpy().view(np.uint32), pos[o_perm].view(np.uint32))
+    del cs, perm, srt, o_perm
+    per, glob = _check_accel(oracle_mod, a, pos, w.box, w.eps, targets=t, label="config%d sampled" % cfg)
+    print("config %d full size: W = %d, max cell %d, %d sampled targets: per-particle max %.3e, global L2 %.3e"
+          % (cfg, W, st["max_cell_count"], t.size, per, glob))
+    if r17:
+        moved = _r17_sequence(oracle_mod, gpu, sol, d, pos, a, w.box, w.ncell, "config %d" % cfg)
+        assert 0.0 < moved < 0.5
 
 
 def test_config4_full_size_sampled(oracle_mod, gpu):
@@ -366,11 +438,36 @@ def test_config4_full_size_sampled(oracle_mod, gpu):
     _full_config(oracle_mod, gpu, 4, 768, 768)
 
 
-@pytest.mark.full
-@pytest.mark.skipif(os.environ.get("SRPP_FULL") != "1", reason="set SRPP_FULL=1 (minutes of GPU + host time)")
-@pytest.mark.parametrize("cfg", [3, 5])
-def test_configs_3_5_full_size_sampled(oracle_mod, gpu, cfg):
-    _full_config(oracle_mod, gpu, cfg, 512, 512)
+def test_config3_full_size_sampled(oracle_mod, gpu):
+    """BASELINE.json configs[2] (256^3, 4000 halos) at full size, sampled targets."""
+    _full_config(oracle_mod, gpu, 3, 512, 512)
+
+
+def test_config5_full_size_force_kick_stream_rebin(oracle_mod, gpu):
+    """BASELINE.json configs[4] as worded: 512^3 strongly clustered particles (3 x 8-bit digit plan at 2^27 elements,
+    4.1 M cells, a multi-million-particle cell), one force evaluation (sampled targets against the oracle) plus
+    re-binning after a kick (the R17 sequence, bit-exact)."""
+    _full_config(oracle_mod, gpu, 5, 384, 384, r17=True)
+
+
+def test_r17_force_kick_stream_rebin_scaled(oracle_mod, gpu):
+    """The R17 sequence at a size the oracle checks in full: force -> kick(tau) -> stream(tau) -> re-bin."""
+    torch, binding = gpu
+    ncell = (12, 10, 14)
+    pos, box = workloads.scaled_clustered(400000, ncell, seed=17, frac_halo=0.8, n_halo=40, a_range=(0.2, 2.5))
+    sol = _solver(gpu, box, ncell, 0.02, pos.shape[0])
+    d = torch.from_numpy(pos).cuda()
+    sol.build_mesh(d)
+    acc = sol.accel()
+    torch.cuda.synchronize()
+    a = acc.cpu().numpy()
+    _check_accel(oracle_mod, a, pos, box, 0.02, label="r17 scaled")
+    moved = _r17_sequence(oracle_mod, gpu, sol, d, pos, a, box, ncell, "scaled")
+    assert 0.0 < moved < 0.5
+    # and the force on the re-binned mesh is still the oracle's
+    a2 = sol.accel()
+    torch.cuda.synchronize()
+    _check_accel(oracle_mod, a2.cpu().numpy(), d.cpu().numpy(), box, 0.02, label="r17 scaled, after re-bin")
 
 
 # ---------------------------------------- open axes and active/passive particles (overloaded node volume) --
@@ -439,6 +536,8 @@ def test_overloaded_subvolume_reproduces_periodic_box(oracle_mod, gpu):
     ref, st = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, 0.05), targets=active_full, stats=True)
     # the shifted coordinates differ from the originals by an fp32 rounding, so allow twice the usual global bar
     per, glob = oracle_mod.error_norms(a[active_sub], ref, st["allowance"])
+    print("overloaded slab vs periodic box: per-particle max %.3e (bar %.0e), global L2 %.3e (bar %.0e)"
+          % (per.max(), PER_PARTICLE_TOL, glob, 2 * GLOBAL_L2_TOL))
     assert per.max() <= PER_PARTICLE_TOL and glob <= 2 * GLOBAL_L2_TOL, (per.max(), glob)
 
 
@@ -512,6 +611,22 @@ def test_new_entry_points_reject_bad_arguments(gpu):
     with pytest.raises(binding.SrppError) as e:
         sol.set_boundary((1, 1, 1), (float("nan"), 0.0, 0.0), (4.0, 32.0, 32.0))
     assert e.value.status == -1
+    # a rejected srpp_set_boundary leaves the previous boundary in place (all three axes validated first)
+    p0 = torch.rand((100, 4), device="cuda") * 31
+    sol.set_boundary((0, 1, 1))
+    sol.build_mesh(p0)
+    a_open = sol.accel().clone()
+    with pytest.raises(binding.SrppError):
+        sol.set_boundary((1, 1, 1), (0.0, 0.0, 9.0), (32.0, 32.0, 5.0))       # bad z only: x must stay open
+    assert torch.equal(sol.accel(), a_open)
+    sol.set_boundary((1, 1, 1))
+    # misaligned float4 pointers: a status code, not a sticky CUDA fault
+    buf = torch.zeros(4 * 101, device="cuda")
+    assert sol.lib.srpp_build_mesh(sol._ctx, buf.data_ptr() + 4, 100) == -1
+    assert sol.lib.srpp_accel(sol._ctx, buf.data_ptr() + 8) == -1
+    assert sol.lib.srpp_kick(sol._ctx, buf.data_ptr() + 4, buf.data_ptr(), C.c_float(0.1), 100) == -1
+    assert sol.lib.srpp_stream(sol._ctx, buf.data_ptr(), buf.data_ptr() + 4, C.c_float(0.1), 100) == -1
+    torch.cuda.synchronize()
     pos = torch.rand((100, 4), device="cuda")
     with pytest.raises(binding.SrppError) as e:
         sol.mbp(pos, [0, 60, 40, 100])                                        # not monotone
