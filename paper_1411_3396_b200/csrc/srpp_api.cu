@@ -19,12 +19,9 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
   const size_t o_flags = take(sizeof(DevFlags));
-  const size_t o_k0 = take(4 * nn), o_k1 = take(4 * nn), o_v0 = take(4 * nn), o_v1 = take(4 * nn);
-  int sp = 0, sb = 0;
-  plan_sort((int32_t)ncells, &sp, &sb);
-  const size_t o_hist = take(4 * ((size_t)1 << sb) * (nn / kSortTile + 1));   // [tiles][bins]
-  const size_t o_coltot = take(4 * (size_t)kSortMaxBins);
-  const size_t o_colpart = take(4 * (size_t)kSortMaxBins * 16);
+  const size_t o_v0 = take(4 * nn), o_v1 = take(4 * nn), o_keys = take(4 * nn);
+  const size_t o_ctl = take(sort_ctl_bytes());
+  const size_t o_status = take(8 * (size_t)kSortMaxBins * (nn / kPassTile + 1));   // [tiles][bins] look-back words
   const size_t o_cs = take(4 * (ncells + 1));
   const size_t o_sorted = take(16 * nn);
   const size_t o_prefix = take(8 * (ncells + 1));
@@ -33,12 +30,11 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   if (c) {
     char* b = c->ws;
     c->flags = (DevFlags*)(b + o_flags);
-    c->keys[0] = (uint32_t*)(b + o_k0); c->keys[1] = (uint32_t*)(b + o_k1);
     c->vals[0] = (uint32_t*)(b + o_v0); c->vals[1] = (uint32_t*)(b + o_v1);
-    c->keys_raw = c->keys[1];
-    c->hist = (uint32_t*)(b + o_hist);
-    c->coltot = (uint32_t*)(b + o_coltot);
-    c->colpart = (uint32_t*)(b + o_colpart);
+    c->sorted_keys_buf = (uint32_t*)(b + o_keys);
+    c->sort_ctl = (uint32_t*)(b + o_ctl);
+    if (c->sort_status != (unsigned long long*)(b + o_status)) c->status_n = 0;   // the array moved: clear before use
+    c->sort_status = (unsigned long long*)(b + o_status);
     c->cell_start = (uint32_t*)(b + o_cs);
     c->sorted = (float4*)(b + o_sorted);
     c->item_prefix = (unsigned long long*)(b + o_prefix);

@@ -16,10 +16,13 @@ constexpr int kSortThreads = 512;             // 16 warps
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortItems = 8;                 // a warp handles 8 steps of 32 consecutive elements
 constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 elements per tile
+constexpr int kPassTile = 4096;               // elements per tile of a digit pass (k_sort_pass)
 constexpr int kSortMinDigitBits = 5;          // >= 32 bins (one warp-row of the column scan)
 constexpr int kSortMaxDigitBits = 8;          // <= 256 bins: >= 16 elements per bin and tile, so the per-digit runs cover whole 32-byte sectors
 constexpr int kSortMaxBins = 1 << kSortMaxDigitBits;
-constexpr int kSortBinsPerThread = kSortMaxBins > kSortThreads ? kSortMaxBins / kSortThreads : 1;
+constexpr int kSortMaxPasses = 3;             // 3 x 8 bits cover the 2^24-cell limit
+// sort control block: 64 words of tile tickets (one per pass) + the global digit histograms [passes][kSortMaxBins]
+constexpr size_t sort_ctl_bytes() { return sizeof(uint32_t) * (64 + (size_t)kSortMaxPasses * kSortMaxBins); }
 
 constexpr int kForceThreads = 256;            // 8 autonomous warps per CTA
 constexpr int kForceWarps = kForceThreads / 32;
@@ -84,12 +87,12 @@ struct srpp_ctx {
   char* ws;
   size_t ws_bytes;
   srpp::DevFlags* flags;
-  uint32_t* keys[2];
-  uint32_t* vals[2];
-  uint32_t* keys_raw;        // cell ids in input order (aliases keys[1]: dead before pass 1 writes it)
-  uint32_t* hist;            // [tiles][nbins] per-tile digit histogram, scanned over tiles in place
-  uint32_t* coltot;          // [nbins] digit totals
-  uint32_t* colpart;         // [slices][nbins] slice totals of the column scan
+  uint32_t* vals[2];         // original indices, ping-pong (unequal masses) / perm of the last pass
+  uint32_t* sorted_keys_buf; // cell ids in sorted order, written by the last pass
+  uint32_t* sort_ctl;        // tile tickets + global digit histograms (cleared by every build)
+  unsigned long long* sort_status;  // [tiles][kSortMaxBins] look-back status words, epoch-tagged
+  int64_t status_n;          // n the status array was last cleared for (0 = never)
+  uint32_t sort_epoch;       // tag of the last pass launched
   float4* pos_tmp;           // payload ping-pong buffer (aliases acc64: mesh build and accel never overlap)
   uint32_t* cell_start;      // [ncells+1]
   float4* sorted;            // [n]
