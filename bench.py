@@ -45,23 +45,39 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+FORCE_PROFILE = os.path.join("profiles", "r02_force_config4_ncu_full.txt")
+FORCE_SOURCE = os.path.join("paper_1411_3396_b200", "csrc", "srpp_force.cu")
+
+
+def _git_blob_hash(path):
+    """git's blob hash of a file (sha1 of 'blob <len>\0' + content), computed without calling git."""
+    import hashlib
+    with open(path, "rb") as fh:
+        data = fh.read()
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
 def _profiled_traffic():
     """DRAM bytes per launch of the force kernel from the committed `ncu --set full` summary under profiles/
-    (dram__bytes_read.sum + dram__bytes_write.sum; text file, never executed).  None if the summary is absent."""
-    path = os.path.join(ROOT, "profiles", "r01_force_config4_ncu_full.txt")
+    (dram__bytes_read.sum + dram__bytes_write.sum; text file, never executed), plus the git blob hash of srpp_force.cu
+    the capture was made from (its header line `source-blob: <hash>`) and whether the shipped source still has it."""
+    path = os.path.join(ROOT, FORCE_PROFILE)
     unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
-    total, seen = 0.0, 0
+    total, seen, blob = 0.0, 0, None
     try:
         with open(path) as fh:
             for line in fh:
+                if line.startswith("source-blob:"):
+                    blob = line.split(":", 1)[1].strip()
                 for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
                     if line.startswith(key + " ["):
                         u = line.split("[")[1].split("]")[0]
                         total += float(line.split("=")[1]) * unit[u]
                         seen += 1
     except OSError:
-        return None
-    return total if seen == 2 else None
+        return None, None, None
+    cur = _git_blob_hash(os.path.join(ROOT, FORCE_SOURCE))
+    return (total if seen == 2 else None), blob, (blob == cur)
 
 
 # --------------------------------------------------------------------------------------- clocks --
@@ -166,11 +182,15 @@ def oracle_rate(oracle, pos, w, budget_s: float, seed: int = 0):
     n_b = int(np.searchsorted(csum, budget_s / per_cand)) + 1
     n_b = int(min(max(n_b, 2 * n_a), t_all.shape[0]))
     t0 = time.perf_counter()
-    oracle.accel(pos, prm, targets=t_all[:n_b])
+    _, st_b = oracle.accel(pos, prm, targets=t_all[:n_b], stats=True)
     t_b = time.perf_counter() - t0
+    # in-cutoff share of the candidate pairs, W-weighted: for targets drawn with probability proportional to their
+    # candidate count, E[n_in_i / cand_i] = sum_i n_in_i / W exactly (the work-weighted half of the sample)
+    wt = order[:n_b] >= (4096 - 4096 // 2)
+    frac_in = float(np.mean(st_b["n_in"][wt] / np.maximum(cand_all[:n_b][wt], 1))) if wt.any() else None
     d_c = int(cand_all[:n_b].sum() - cand_all[:n_a].sum())
     rate = d_c / max(t_b - t_a, 1e-9)
-    return {"value": rate, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+    return {"value": rate, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "in_cutoff_fraction": frac_in,
             "sample": "%s: %d targets (half uniform, half work-weighted; SURVEY.md 8(d)), %d chaining-mesh candidate "
                       "pairs in %.1f s of fp64 oracle time; marginal rate between nested samples of %d and %d targets "
                       "(fixed cell-list build of %.1f s per call excluded)"
@@ -299,6 +319,7 @@ def run_product(args, w):
         return
 
     peaks, peak_kind = _peaks()
+    traffic, traffic_blob, traffic_ok = _profiled_traffic()
     props = torch.cuda.get_device_properties(dev)
     sms = props.multi_processor_count
     clk = clocks.summary()
@@ -324,9 +345,10 @@ def run_product(args, w):
         "clocks": clk, "e2e": e2e, "gpu_launches": launches,
         "roofline": {"bound": "alu", "kernel": "k_pp_force", "achieved": achieved, "peak": peak_tflops,
                      "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None,
-                     "traffic": _profiled_traffic() if args.config == 4 else None,
-                     "traffic_kind": "DRAM bytes per launch, ncu --set full capture in profiles/ (the kernel is ALU-bound: "
-                                     "algorithmic bytes are 2 x 16 B x N + cell tables, re-reads are served by L2)",
+                     "traffic": traffic if args.config == 4 else None,
+                     "traffic_kind": "DRAM bytes per launch, ncu --set full capture %s (the kernel is ALU-bound: "
+                                     "algorithmic bytes are 2 x 16 B x N + cell tables, re-reads are served by L2)" % FORCE_PROFILE,
+                     "traffic_capture_source_blob": traffic_blob, "traffic_capture_matches_shipped_source": traffic_ok,
                      "peak_kind": "nominal: %d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (sm_max_mhz, %s); "
                                   "30 flop per candidate pair" % (sms, f_max_hz / 1e6, peak_kind),
                      "launch_ms": force_avg_ms, "fp32_probe": probe,
@@ -341,9 +363,97 @@ def run_product(args, w):
     if world == 1 and not args.no_cpu_baseline:
         import oracle                                  # cpu_baseline leg: the one place the product arm may run it
         oracle.build()
-        line["cpu_baseline"] = oracle_rate(oracle, pos, w, args.cpu_budget)
+        cb = oracle_rate(oracle, pos, w, args.cpu_budget)
+        line["cpu_baseline"] = cb
+        # oracle binning timed in full; in-cutoff pairs beside candidate pairs; the full-config oracle
+        # time as a labelled extrapolation
+        t0 = time.perf_counter()
+        oracle.build_mesh(pos, w.box, w.ncell)
+        line["phases"]["oracle_mesh_ms"] = 1e3 * (time.perf_counter() - t0)
+        line["phases"]["oracle_mesh_kind"] = "orc_build_mesh, all %d particles, one host thread (plain counting sort)" % n
+        frac = cb.pop("in_cutoff_fraction")
+        line["in_cutoff"] = {"fraction_of_candidates": frac, "pairs_per_s": value * frac,
+                             "kind": "mean of n_in_i / candidates_i over the oracle's work-weighted target sample (= sum n_in / W in expectation)"}
+        cb["full_config_extrapolated_s"] = W / cb["value"]
+        cb["full_config_extrapolated_kind"] = "EXTRAPOLATION: W / marginal oracle rate, not a measured run"
+    if world == 1 and not args.no_extras:
+        del d_pos, d_acc, d_vel, sol
+        torch.cuda.empty_cache()
+        line["other"] = run_extras(args, torch, binding, dev, peak_tflops, peaks)
     print(json.dumps(line), flush=True)
     rep.close()
+
+
+def run_extras(args, torch, binding, dev, peak_tflops, peaks):
+    """Short device-timed passes that are NOT the headline (outside its timed region): BASELINE.json configs 1-3
+    (force fraction of FP32 peak, binning GB/s), the sub-cycle call, and srpp_mbp with its own roofline."""
+    out = {}
+    for cfg, reps in ((1, 20), (2, 10), (3, 1)):
+        wc = workloads.CONFIGS[cfg]
+        pos = workloads.generate(wc)
+        n = pos.shape[0]
+        sol = binding.Solver(wc.box, wc.ncell, wc.rcut, wc.eps, n_max=n, device=dev)
+        sol.set_timing(True)
+        d_pos = torch.from_numpy(pos).to(dev)
+        d_acc = torch.empty_like(d_pos)
+        sol.build_mesh(d_pos); sol.accel(d_acc)                        # warm-up
+        mesh, force, accel = [], [], []
+        for _ in range(reps):
+            sol.build_mesh(d_pos)
+            sol.accel(d_acc)
+            t = sol.get_timings()
+            mesh.append(t["mesh_ms"]); force.append(t["force_ms"]); accel.append(t["accel_ms"])
+        st = sol.get_stats()
+        W = st["candidate_pairs"]
+        ncells = wc.ncell[0] * wc.ncell[1] * wc.ncell[2]
+        fm, mm = float(np.median(force)), float(np.median(mesh))
+        rec = {"workload": wc.name, "n_particles": n, "candidate_pairs_W": W, "reps": reps, "force_ms": fm,
+               "accel_ms": float(np.median(accel)), "mesh_ms": mm,
+               "pairs_per_s_force_kernel": W / (fm * 1e-3),
+               "frac_of_fp32_peak": FLOP_PER_PAIR * W / (fm * 1e-3) / 1e12 / peak_tflops,
+               "pair_slots_per_candidate_pair": st["pair_slots"] / max(W, 1),
+               "binning_gbs": (BIN_BYTES_PER_PARTICLE * n + 8 * ncells) / (mm * 1e-3) / 1e9}
+        rec["binning_frac_of_hbm"] = rec["binning_gbs"] / peaks["hbm_gbs"]
+        if cfg == 2:   # the sub-cycle call (PAPER.md:73): stream - accel - kick - stream, re-bin included
+            d_vel = torch.zeros_like(d_pos)
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            sol.subcycle(d_pos, d_vel, 1e-3, 1e-3, 1, acc=d_acc)
+            torch.cuda.synchronize()
+            ev0.record()
+            sol.subcycle(d_pos, d_vel, 1e-3, 1e-3, 4, acc=d_acc)
+            ev1.record()
+            torch.cuda.synchronize()
+            rec["subcycle_ms_per_substep"] = ev0.elapsed_time(ev1) / 4
+            del d_vel
+        out["config%d" % cfg] = rec
+        del sol, d_pos, d_acc
+        torch.cuda.empty_cache()
+    # most bound particle (PAPER.md:93-97: the paper's Thrust version ran 45x faster on K20X than on the CPU; context)
+    rng = np.random.default_rng(7)
+    sizes = [2_000_000] + [200_000] * 10 + [2000] * 500
+    tot = int(sum(sizes))
+    hs = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    p = np.ones((tot, 4), dtype=np.float32)
+    p[:, :3] = rng.normal(0, 1.0, (tot, 3)).astype(np.float32) + np.repeat(rng.uniform(10, 500, (len(sizes), 3)), sizes, axis=0).astype(np.float32)
+    sol = binding.Solver((512.0,) * 3, (16,) * 3, 3.0, 0.05, n_max=16, device=dev)
+    d = torch.from_numpy(p).to(dev)
+    sol.mbp(d, hs, want_phi=False)
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(3):
+        sol.mbp(d, hs, want_phi=False)
+    ev1.record()
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / 3
+    pairs = float(sum(float(k) * float(k) for k in sizes))
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    xu_peak = sms * 16 * 1e6 * float(peaks.get("sm_max_mhz") or 1965.0)       # one MUFU.RSQ per pair, 16 per SM and clock
+    out["mbp"] = {"halos": len(sizes), "members": tot, "ordered_pairs": pairs, "ms": ms, "pairs_per_s": pairs / (ms * 1e-3),
+                  "roofline": {"bound": "xu", "peak_pairs_per_s": xu_peak, "frac": pairs / (ms * 1e-3) / xu_peak,
+                               "peak_kind": "%d SMs x 16 MUFU.RSQ per clock x sm_max_mhz, one rsqrt per pair (DESIGN.md 5.4)" % sms},
+                  "paper_context": "PAPER.md:97: the PISTON/Thrust centre finder ran ~45x faster on a K20X than on the CPU"}
+    return out
 
 
 def main():
@@ -357,6 +467,7 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--ref-budget", type=float, default=150.0, help="seconds for the whole --impl reference run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the configs 1-3 / sub-cycle / MBP passes")
     ap.add_argument("--no-phase-timing", dest="phase_timing", action="store_false")
     args = ap.parse_args()
     w = workloads.CONFIGS[args.config]

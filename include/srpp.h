@@ -41,11 +41,14 @@ extern "C" {
 
 typedef enum {
   SRPP_OK = 0,
-  SRPP_ERR_INVALID_ARG = -1, /* null pointer, n < 0 or n >= 2^31, eps <= 0, rcut <= 0, non-finite parameter   */
-  SRPP_ERR_GEOMETRY = -2,    /* ncell < 3 on an axis, box/ncell < rcut, or more than 2^24 cells (R8)          */
+  SRPP_ERR_INVALID_ARG = -1, /* null or misaligned (16 B) pointer, n < 0 or n >= 2^31, eps <= 0, rcut <= 0,
+                                non-finite parameter                                                         */
+  SRPP_ERR_GEOMETRY = -2,    /* ncell < 3 on an axis, box/ncell < rcut, more than 2^24 cells (R8), or a box
+                                length / cutoff above 2^24 grid units (fp32 exact-integer range)              */
   SRPP_ERR_DOMAIN = -3,      /* a position outside [0, L) or not finite, found while binning (R13)            */
   SRPP_ERR_WORKSPACE = -4,   /* workspace too small or not 256-byte aligned                                   */
-  SRPP_ERR_STATE = -5,       /* srpp_accel before a successful srpp_build_mesh, or n mismatch                 */
+  SRPP_ERR_STATE = -5,       /* srpp_accel before a successful srpp_build_mesh, n mismatch, or the current CUDA
+                                device is not the one the context was created on                             */
   SRPP_ERR_CUDA = -6         /* CUDA runtime error (text of the last one: srpp_last_cuda_error)                */
 } srpp_status;
 
@@ -148,13 +151,15 @@ int32_t srpp_set_boundary(srpp_ctx* ctx, const int32_t* periodic_host, const flo
  *     phi_i = - sum_{j in h, j != i} m_j / sqrt(|x_j - x_i|^2 + eps^2)        (G = 1, eps of srpp_params, plain differences)
  * The centre is the member with the smallest phi (lowest index on ties).
  *   pos_mass          device float4[n]; positions need not lie in the box (no mesh is used)
- *   halo_start_host   HOST int64[nhalo+1], non-decreasing, within [0, n]; read during the call
+ *   halo_start_host   HOST int64[nhalo+1], non-decreasing, within [0, n]; read (validated and uploaded) during the
+ *                     call; nhalo <= 2^24
  *   phi               device float[n] or NULL: phi of every halo member (entries outside every halo are not written)
  *   mbp_index         device int64[nhalo]: index into pos_mass of each halo's centre, -1 for an empty halo
  *   mbp_phi           device float[nhalo] or NULL: its potential (0 for an empty halo)
  *   workspace         device, 256-byte aligned, >= srpp_mbp_workspace_bytes(n, nhalo); owned by the caller
- * Pair arithmetic in fp32 (partial sums of <= 1024 terms folded in fp64).  Asynchronous on the context's stream after
- * the halo table has been uploaded.  Errors: INVALID_ARG, WORKSPACE, CUDA. */
+ * Pair arithmetic in fp32 (partial sums of <= 1024 terms folded in fp64; the argmin is taken on those fp64 sums).
+ * Asynchronous on the context's stream: the item prefix is computed on the device, no synchronisation.
+ * Errors: INVALID_ARG, WORKSPACE, STATE (another device is current), CUDA. */
 int32_t srpp_mbp_workspace_bytes(int64_t n, int64_t nhalo, size_t* bytes_host);
 int32_t srpp_mbp(srpp_ctx* ctx, const float* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
                  float* phi, int64_t* mbp_index, float* mbp_phi, void* workspace, size_t workspace_bytes);
@@ -166,6 +171,19 @@ int32_t srpp_kick(srpp_ctx* ctx, float* vel, const float* acc, float kdt, int64_
 /* Stream (drift): x <- wrap(fmaf(v, dt, x)) per component in fp32, result in [0, L) (a value that rounds
  * to L becomes 0; R13, R17).  Requires |v*dt| < L.  pos_mass is updated in place.  Asynchronous. */
 int32_t srpp_stream(srpp_ctx* ctx, float* pos_mass, const float* vel, float dt, int64_t n);
+
+/* The short-range sub-cycle as one call ("short-range force timestep": evolve, update the active
+ * particles, stream the passive ones; reading R20 in DESIGN.md): nsub times
+ *     x <- stream(x, v, dt/2);   a = accel(x);   v <- kick(v, a, kdt);   x <- stream(x, v, dt/2)
+ * with srpp_stream / srpp_build_mesh + srpp_accel / srpp_kick semantics for the three pieces (dt/2 = the fp32 product
+ * 0.5f*dt; with an active box set by srpp_set_boundary the passive particles have a = 0 and are only streamed).
+ *   pos_mass, vel   device float4[n], updated in place
+ *   acc             device float4[n]: accelerations of the LAST sub-step, caller's order (.w = 0)
+ * On return the chaining mesh held by the context is the mesh of the RETURNED positions (srpp_get_mesh, or a following
+ * srpp_accel / srpp_subcycle, may use it).  Synchronises the stream (domain check of every re-bin).
+ * Errors: INVALID_ARG (null / misaligned pointer, nsub < 0, non-finite dt or kdt), WORKSPACE, DOMAIN, STATE, CUDA. */
+int32_t srpp_subcycle(srpp_ctx* ctx, float* pos_mass, float* vel, float* acc, float dt, float kdt, int32_t nsub,
+                      int64_t n);
 
 /* End-to-end convenience for callers holding HOST arrays: copies pos_mass_host[4n] (and vel_host[4n] if
  * not NULL) to the device, builds the mesh, computes accelerations, optionally kicks (vel_host != NULL:

@@ -20,7 +20,7 @@ STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "GEOMETRY", -3: "DOMAIN", -4: "W
 EXPORTS = ("srpp_version", "srpp_default_poly", "srpp_workspace_bytes", "srpp_create", "srpp_destroy",
            "srpp_build_mesh", "srpp_get_mesh", "srpp_accel", "srpp_get_stats", "srpp_kick", "srpp_stream",
            "srpp_step_host", "srpp_strerror", "srpp_last_cuda_error", "srpp_set_timing", "srpp_get_timings",
-           "srpp_probe_fp32", "srpp_set_boundary", "srpp_mbp_workspace_bytes", "srpp_mbp")
+           "srpp_probe_fp32", "srpp_set_boundary", "srpp_mbp_workspace_bytes", "srpp_mbp", "srpp_subcycle")
 
 
 class SrppParams(C.Structure):
@@ -78,6 +78,8 @@ def load() -> C.CDLL:
     L.srpp_kick.argtypes = [vp, vp, vp, f32, i64]
     L.srpp_stream.restype = i32
     L.srpp_stream.argtypes = [vp, vp, vp, f32, i64]
+    L.srpp_subcycle.restype = i32
+    L.srpp_subcycle.argtypes = [vp, vp, vp, vp, f32, f32, i32, i64]
     L.srpp_step_host.restype = i32
     L.srpp_step_host.argtypes = [vp, vp, vp, vp, f32, i64, vp, C.c_size_t]
     L.srpp_set_timing.restype = i32
@@ -285,6 +287,24 @@ class Solver:
         self._check(self.lib.srpp_stream(self._ctx, pos_mass.data_ptr(), vel.data_ptr(), float(dt), vel.shape[0]),
                     "srpp_stream")
         return pos_mass
+
+    def subcycle(self, pos_mass, vel, dt: float, kdt: float = None, nsub: int = 1, acc=None):
+        """srpp_subcycle: nsub x {stream(dt/2), accel, kick(kdt), stream(dt/2)}; pos_mass and vel are updated in place.
+        Returns acc (accelerations of the last sub-step).  kdt defaults to dt."""
+        torch = self._torch
+        self._f4(pos_mass, "pos_mass"), self._f4(vel, "vel")
+        if vel.shape != pos_mass.shape:
+            raise ValueError("pos_mass and vel shapes differ")
+        n = pos_mass.shape[0]
+        if acc is None:
+            acc = torch.zeros((n, 4), dtype=torch.float32, device=self.device)
+        self._f4(acc, "acc")
+        self.n = -1
+        self._check(self.lib.srpp_subcycle(self._ctx, pos_mass.data_ptr(), vel.data_ptr(), acc.data_ptr(), float(dt),
+                                           float(dt if kdt is None else kdt), int(nsub), n), "srpp_subcycle")
+        self.n = n
+        self._pos_ref = pos_mass
+        return acc
 
     def step_host(self, pos_mass_host, vel_host, acc_host, kdt: float, scratch):
         """End-to-end call on HOST (ideally pinned) float32 [n,4] tensors/arrays; `scratch` is a CUDA uint8 tensor

@@ -358,6 +358,24 @@ int32_t srpp_stream(srpp_ctx* c, float* pos_mass, const float* vel, float dt, in
   return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
 }
 
+int32_t srpp_subcycle(srpp_ctx* c, float* pos_mass, float* vel, float* acc, float dt, float kdt, int32_t nsub, int64_t n) {
+  if (!c || n < 0 || n >= ((int64_t)1 << 31) || nsub < 0 || !isfinite(dt) || !isfinite(kdt) ||
+      (n > 0 && (!pos_mass || !vel || !acc)) || misaligned16(pos_mass) || misaligned16(vel) || misaligned16(acc))
+    return SRPP_ERR_INVALID_ARG;
+  if (const int32_t d = check_device(c)) return d;
+  const float half = 0.5f * dt;            // exact in fp32
+  int32_t rc = SRPP_OK;
+  for (int32_t s = 0; s < nsub; ++s) {
+    if ((rc = srpp_stream(c, pos_mass, vel, half, n)) != SRPP_OK) return rc;
+    if ((rc = srpp_build_mesh(c, pos_mass, n)) != SRPP_OK) return rc;
+    if ((rc = srpp_accel(c, acc)) != SRPP_OK) return rc;
+    if ((rc = srpp_kick(c, vel, acc, kdt, n)) != SRPP_OK) return rc;
+    if ((rc = srpp_stream(c, pos_mass, vel, half, n)) != SRPP_OK) return rc;
+  }
+  // the context's mesh is the mesh of the returned positions
+  return srpp_build_mesh(c, pos_mass, n);
+}
+
 int32_t srpp_step_host(srpp_ctx* c, const float* pos_mass_host, float* vel_host, float* acc_host, float kdt,
                        int64_t n, void* device_scratch, size_t device_scratch_bytes) {
   if (!c || n < 0 || n >= ((int64_t)1 << 31) || (n > 0 && (!pos_mass_host || !acc_host || !device_scratch))) return SRPP_ERR_INVALID_ARG;

@@ -346,6 +346,107 @@ def test_subcycle_fixed_positions(oracle_mod, gpu):
     assert glob < GLOBAL_L2_TOL and per.max() < PER_PARTICLE_TOL
 
 
+def _subcycle_case(seed=51, n=60000, ncell=(6, 5, 7), eps=0.05):
+    pos, box = workloads.scaled_clustered(n, ncell, seed=seed, frac_halo=0.6, n_halo=8, a_range=(0.3, 1.5))
+    rng = np.random.default_rng(seed)
+    vel = np.zeros_like(pos)
+    vel[:, :3] = rng.normal(0, 0.5, (pos.shape[0], 3)).astype(np.float32)
+    return pos, vel, box, ncell, eps
+
+
+def test_subcycle_step_by_step(oracle_mod, gpu):
+    """srpp_subcycle (R20), one sub-step per call, three calls.  Each call is checked against the oracle
+    started from the GPU's own state: the accelerations within the R18 bars at the mid-step positions, velocities and
+    positions BIT-EXACT against orc_stream / orc_kick fed the GPU's accelerations (the composition and its order), and
+    the mesh the context holds afterwards bit-exact against orc_build_mesh of the returned positions."""
+    torch, binding = gpu
+    pos, vel, box, ncell, eps = _subcycle_case()
+    n = pos.shape[0]
+    sol = binding.Solver(box, ncell, 3.0, eps, n_max=n)
+    d_pos, d_vel = torch.from_numpy(pos.copy()).cuda(), torch.from_numpy(vel.copy()).cuda()
+    dt, kdt = 0.004, 0.003
+    prm = oracle_mod.make_params(box, 3.0, eps)
+    x0, v0 = pos, vel
+    for step in range(3):
+        acc = sol.subcycle(d_pos, d_vel, dt, kdt, 1)
+        torch.cuda.synchronize()
+        a, x1, v1 = acc.cpu().numpy(), d_pos.cpu().numpy(), d_vel.cpu().numpy()
+        half = np.float32(0.5) * np.float32(dt)
+        x_mid = oracle_mod.stream(x0, v0, half, box)
+        ref, st = oracle_mod.accel(x_mid, prm, stats=True)
+        per, glob = oracle_mod.error_norms(a, ref, st["allowance"])
+        assert per.max() <= PER_PARTICLE_TOL and glob <= GLOBAL_L2_TOL, (step, per.max(), glob)
+        v_exp = oracle_mod.kick(v0, a, kdt)
+        assert np.array_equal(v1.view(np.uint32), v_exp.view(np.uint32)), step
+        x_exp = oracle_mod.stream(x_mid, v_exp, half, box)
+        assert np.array_equal(x1.view(np.uint32), x_exp.view(np.uint32)), step
+        cs, perm, srt = (t.cpu().numpy() for t in sol.get_mesh())
+        o_cs, o_perm, o_srt = oracle_mod.build_mesh(x1, box, ncell)
+        assert np.array_equal(cs.view(np.uint32), o_cs) and np.array_equal(perm.view(np.uint32), o_perm), step
+        assert np.array_equal(srt.view(np.uint32), o_srt.view(np.uint32)), step
+        moved = np.mean(oracle_mod.cell_ids(x0, box, ncell) != oracle_mod.cell_ids(x1, box, ncell))
+        print("sub-step %d: %.2f %% of the particles changed cell; accel per-particle %.2e, L2 %.2e"
+              % (step, 100 * moved, per.max(), glob))
+        # the mesh is valid: a plain srpp_accel right after needs no re-build
+        a2 = sol.accel().cpu().numpy()
+        ref2, st2 = oracle_mod.accel(x1, prm, stats=True)
+        per2, glob2 = oracle_mod.error_norms(a2, ref2, st2["allowance"])
+        assert per2.max() <= PER_PARTICLE_TOL and glob2 <= GLOBAL_L2_TOL
+        x0, v0 = x1, v1
+
+
+def test_subcycle_several_substeps_vs_oracle(oracle_mod, gpu):
+    """nsub = 4 in one call against orc_subcycle from the same start: the trajectories differ only by the fp32-vs-fp64
+    rounding of the accelerations (1e-6 relative), far below the per-step changes."""
+    torch, binding = gpu
+    pos, vel, box, ncell, eps = _subcycle_case(seed=52, n=40000, ncell=(5, 5, 6))
+    n = pos.shape[0]
+    sol = binding.Solver(box, ncell, 3.0, eps, n_max=n)
+    d_pos, d_vel = torch.from_numpy(pos.copy()).cuda(), torch.from_numpy(vel.copy()).cuda()
+    dt = 0.002
+    acc = sol.subcycle(d_pos, d_vel, dt, dt, 4)
+    torch.cuda.synchronize()
+    xo, vo, ao = oracle_mod.subcycle(pos, vel, oracle_mod.make_params(box, 3.0, eps), dt, dt, 4)
+    x, v, a = d_pos.cpu().numpy(), d_vel.cpu().numpy(), acc.cpu().numpy()
+    dv_step = np.abs(vo[:, :3] - vel[:, :3]).max()
+    assert dv_step > 1e-2
+    d = x[:, :3].astype(np.float64) - xo[:, :3]
+    d -= np.asarray(box) * np.round(d / np.asarray(box))
+    print("4 sub-steps: max |dx| %.2e, max |dv| %.2e (kick size %.2e)" % (np.abs(d).max(), np.abs(v[:, :3] - vo[:, :3]).max(), dv_step))
+    assert np.abs(v[:, :3] - vo[:, :3]).max() <= 2e-5 * dv_step + 1e-6
+    assert np.abs(d).max() <= 2e-5
+    per, glob = oracle_mod.error_norms(a, ao)
+    assert glob <= 1e-4          # accelerations at slightly different positions (the differences above)
+    # nsub = 0: nothing moves, the mesh is (re)built
+    x_before = d_pos.clone()
+    sol.subcycle(d_pos, d_vel, dt, dt, 0)
+    assert torch.equal(x_before, d_pos)
+
+
+def test_subcycle_active_box_streams_passive_particles(oracle_mod, gpu):
+    """active particles are updated, passive ones only streamed."""
+    torch, binding = gpu
+    pos, vel, box, ncell, eps = _subcycle_case(seed=53, n=30000, ncell=(8, 5, 5))
+    sol = binding.Solver(box, ncell, 3.0, eps, n_max=pos.shape[0])
+    sol.set_boundary((0, 1, 1), (3.2 * 2, 0.0, 0.0), (3.2 * 6, box[1], box[2]))
+    vel[:, 0] *= 0.01                                         # keep everybody inside the open x range
+    keep = (pos[:, 0] > 0.5) & (pos[:, 0] < box[0] - 0.5)
+    pos, vel = pos[keep].copy(), vel[keep].copy()
+    d_pos, d_vel = torch.from_numpy(pos.copy()).cuda(), torch.from_numpy(vel.copy()).cuda()
+    dt = 0.004
+    acc = sol.subcycle(d_pos, d_vel, dt, dt, 1)
+    torch.cuda.synchronize()
+    a, v1, x1 = acc.cpu().numpy(), d_vel.cpu().numpy(), d_pos.cpu().numpy()
+    half = np.float32(0.5) * np.float32(dt)
+    x_mid = oracle_mod.stream(pos, vel, half, box)
+    cx = oracle_mod.cell_ids(x_mid, box, ncell) % ncell[0]
+    passive = (cx < 2) | (cx >= 6)
+    assert passive.any() and (~passive).any()
+    assert np.all(a[passive] == 0.0) and np.array_equal(v1[passive], vel[passive])
+    assert np.array_equal(x1[passive], oracle_mod.stream(x_mid, vel, half, box)[passive])
+    assert np.abs(a[~passive, :3]).max() > 0
+
+
 def test_step_host_matches_device_path(oracle_mod, gpu):
     torch, binding = gpu
     pos, box = workloads.scaled_clustered(50000, (6, 5, 7), seed=3, frac_halo=0.5, n_halo=4)
