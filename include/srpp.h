@@ -164,6 +164,41 @@ int32_t srpp_mbp_workspace_bytes(int64_t n, int64_t nhalo, size_t* bytes_host);
 int32_t srpp_mbp(srpp_ctx* ctx, const float* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
                  float* phi, int64_t* mbp_index, float* mbp_phi, void* workspace, size_t workspace_bytes);
 
+/* Block decomposition of the node volume with the x2 adaptive refinement rule (PAPER.md:73-77:
+ * "1) Each node partitions itself into overlapping data blocks, 2) evolves the blocks independently, and 3) reconciles the
+ * alive particles, whereby removing the unnecessary duplicated passive ones"; "the x-axis is equally partitioned in PM
+ * grid units"; a block whose "timing is more than a factor of two larger than the average" is "divided a factor of two
+ * finer").  One GPU evaluates the blocks one after the other; each block is an independent problem: its particles (the
+ * active x-range plus a passive shell of >= rcut on both sides, through the periodic face if x is periodic) are extracted
+ * into their own arrays in a block-local frame, get their own chaining mesh with OPEN x faces and their own force
+ * evaluation, and only the active particles' accelerations are written back.
+ *   srpp_blocks_init      (re)starts the plan with nblocks equal x-ranges, boundaries at integer grid units (box[0] must be
+ *                         integer-valued and >= nblocks, else GEOMETRY; 1 <= nblocks <= SRPP_MAX_BLOCKS)
+ *   srpp_accel_blocks     accelerations of all n particles (caller's order, .w = 0), block by block, from the positions
+ *                         given here (the context's own mesh is neither used nor changed).  Every block is timed on the
+ *                         device; afterwards the plan for the NEXT call is refined by the x2 rule.  The y/z periodic flags
+ *                         of srpp_set_boundary apply; its active box does not.  Synchronises per block.
+ *                         workspace: device, 256-byte aligned, >= srpp_blocks_workspace_bytes(params, n).
+ *   srpp_get_blocks       the blocks of the last srpp_accel_blocks (host array), with their device times.
+ * Block-local coordinates are exact in fp32 (integer frame origins) except for the shell that wraps through the face
+ * x = box[0]; results agree with the periodic evaluation within the north_star tolerances (tested).
+ * Errors: INVALID_ARG, GEOMETRY, WORKSPACE, STATE (no plan / other device), DOMAIN, CUDA. */
+#define SRPP_MAX_BLOCKS 64
+typedef struct {
+  float x0, x1;              /* active range [x0, x1), grid units                                                  */
+  int32_t level;             /* refinement level (0 = initial partition)                                           */
+  int32_t pad_;
+  int64_t n_active, n_total; /* active particles / particles incl. the passive shell                               */
+  uint64_t candidate_pairs;  /* W of the block's own mesh (sum over blocks / W of the box = duplicated work)        */
+  float ms;                  /* device time of the block: extract + mesh + force + reconcile                       */
+  float pad2_;
+} srpp_block_info;
+int32_t srpp_blocks_workspace_bytes(const srpp_params* params, int64_t n, size_t* bytes_host);
+int32_t srpp_blocks_init(srpp_ctx* ctx, int32_t nblocks);
+int32_t srpp_accel_blocks(srpp_ctx* ctx, const float* pos_mass, int64_t n, float* acc, void* workspace,
+                          size_t workspace_bytes);
+int32_t srpp_get_blocks(const srpp_ctx* ctx, srpp_block_info* blocks_host, int32_t capacity, int32_t* count_host);
+
 /* A7: sub-cycled kick, v <- fmaf(a, kdt, v) per component in fp32 (R16); .w lanes untouched.
  * vel, acc: device float4[n].  Asynchronous. */
 int32_t srpp_kick(srpp_ctx* ctx, float* vel, const float* acc, float kdt, int64_t n);

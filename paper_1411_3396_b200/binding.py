@@ -20,7 +20,8 @@ STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "GEOMETRY", -3: "DOMAIN", -4: "W
 EXPORTS = ("srpp_version", "srpp_default_poly", "srpp_workspace_bytes", "srpp_create", "srpp_destroy",
            "srpp_build_mesh", "srpp_get_mesh", "srpp_accel", "srpp_get_stats", "srpp_kick", "srpp_stream",
            "srpp_step_host", "srpp_strerror", "srpp_last_cuda_error", "srpp_set_timing", "srpp_get_timings",
-           "srpp_probe_fp32", "srpp_set_boundary", "srpp_mbp_workspace_bytes", "srpp_mbp", "srpp_subcycle")
+           "srpp_probe_fp32", "srpp_set_boundary", "srpp_mbp_workspace_bytes", "srpp_mbp", "srpp_subcycle",
+           "srpp_blocks_workspace_bytes", "srpp_blocks_init", "srpp_accel_blocks", "srpp_get_blocks")
 
 
 class SrppParams(C.Structure):
@@ -31,6 +32,14 @@ class SrppParams(C.Structure):
 class SrppStats(C.Structure):
     _fields_ = [("work_items", C.c_uint64), ("pair_slots", C.c_uint64), ("candidate_pairs", C.c_uint64),
                 ("max_cell_count", C.c_uint32), ("uniform_mass", C.c_uint32), ("kernel_launches", C.c_uint64)]
+
+
+class SrppBlockInfo(C.Structure):
+    _fields_ = [("x0", C.c_float), ("x1", C.c_float), ("level", C.c_int32), ("pad_", C.c_int32), ("n_active", C.c_int64),
+                ("n_total", C.c_int64), ("candidate_pairs", C.c_uint64), ("ms", C.c_float), ("pad2_", C.c_float)]
+
+
+SRPP_MAX_BLOCKS = 64
 
 
 class SrppTimings(C.Structure):
@@ -78,6 +87,14 @@ def load() -> C.CDLL:
     L.srpp_kick.argtypes = [vp, vp, vp, f32, i64]
     L.srpp_stream.restype = i32
     L.srpp_stream.argtypes = [vp, vp, vp, f32, i64]
+    L.srpp_blocks_workspace_bytes.restype = i32
+    L.srpp_blocks_workspace_bytes.argtypes = [C.POINTER(SrppParams), i64, C.POINTER(C.c_size_t)]
+    L.srpp_blocks_init.restype = i32
+    L.srpp_blocks_init.argtypes = [vp, i32]
+    L.srpp_accel_blocks.restype = i32
+    L.srpp_accel_blocks.argtypes = [vp, vp, i64, vp, vp, C.c_size_t]
+    L.srpp_get_blocks.restype = i32
+    L.srpp_get_blocks.argtypes = [vp, C.POINTER(SrppBlockInfo), i32, C.POINTER(i32)]
     L.srpp_subcycle.restype = i32
     L.srpp_subcycle.argtypes = [vp, vp, vp, vp, f32, f32, i32, i64]
     L.srpp_step_host.restype = i32
@@ -287,6 +304,32 @@ class Solver:
         self._check(self.lib.srpp_stream(self._ctx, pos_mass.data_ptr(), vel.data_ptr(), float(dt), vel.shape[0]),
                     "srpp_stream")
         return pos_mass
+
+    def blocks_init(self, nblocks: int) -> None:
+        """srpp_blocks_init: start the block plan with nblocks equal x-ranges."""
+        self._check(self.lib.srpp_blocks_init(self._ctx, int(nblocks)), "srpp_blocks_init")
+
+    def accel_blocks(self, pos_mass, acc=None):
+        """srpp_accel_blocks: accelerations block by block (extract, own mesh, force, reconcile); refines the plan for the
+        next call by the x2 rule.  Returns (acc, blocks) with blocks = list of dicts (srpp_block_info)."""
+        torch = self._torch
+        self._f4(pos_mass, "pos_mass")
+        n = pos_mass.shape[0]
+        if acc is None:
+            acc = torch.empty((n, 4), dtype=torch.float32, device=self.device)
+        self._f4(acc, "acc")
+        nbytes = C.c_size_t(0)
+        self._check(self.lib.srpp_blocks_workspace_bytes(C.byref(self.params), n, C.byref(nbytes)), "srpp_blocks_workspace_bytes")
+        if getattr(self, "_blocks_ws", None) is None or self._blocks_ws.numel() < nbytes.value:
+            self._blocks_ws = torch.empty(int(nbytes.value), dtype=torch.uint8, device=self.device)
+        self._check(self.lib.srpp_accel_blocks(self._ctx, pos_mass.data_ptr(), n, acc.data_ptr(), self._blocks_ws.data_ptr(),
+                                               self._blocks_ws.numel()), "srpp_accel_blocks")
+        info = (SrppBlockInfo * SRPP_MAX_BLOCKS)()
+        cnt = C.c_int32(0)
+        self._check(self.lib.srpp_get_blocks(self._ctx, info, SRPP_MAX_BLOCKS, C.byref(cnt)), "srpp_get_blocks")
+        blocks = [{k: getattr(info[b], k) for k in ("x0", "x1", "level", "n_active", "n_total", "candidate_pairs", "ms")}
+                  for b in range(cnt.value)]
+        return acc, blocks
 
     def subcycle(self, pos_mass, vel, dt: float, kdt: float = None, nsub: int = 1, acc=None):
         """srpp_subcycle: nsub x {stream(dt/2), accel, kick(kdt), stream(dt/2)}; pos_mass and vel are updated in place.

@@ -199,6 +199,7 @@ void srpp_destroy(srpp_ctx* c) {
   if (!c) return;
   for (int i = 0; i < kNumEvents; ++i)
     if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+  free_block_plan(c);
   delete c;
 }
 

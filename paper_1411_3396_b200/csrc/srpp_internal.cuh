@@ -109,6 +109,7 @@ struct srpp_ctx {
   bool ev_mesh_valid, ev_accel_valid;
   uint64_t launches;         // kernels launched by this context so far (harness evidence)
   int mbp_occ;               // resident CTAs per SM of k_mbp_phi (queried once)
+  void* block_plan;          // srpp_blocks.cu: x-partition + last timings (host), nullptr until srpp_blocks_init
 };
 
 namespace srpp {
@@ -130,6 +131,8 @@ cudaError_t launch_scan_u64(cudaStream_t st, unsigned long long* data, int n, un
 size_t mbp_workspace_layout(int64_t n, int64_t nhalo, size_t* o_phi, size_t* o_prefix, size_t* o_start, size_t* o_tmp);
 cudaError_t launch_mbp(srpp_ctx* c, const float4* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
                        float* phi_out, long long* mbp_index, float* mbp_phi, char* ws);
+// srpp_blocks.cu
+void free_block_plan(srpp_ctx* c);
 // srpp_probe.cu
 cudaError_t run_fp32_probe(cudaStream_t st, int variant, int iters, double* flops_per_s, float* checksum);
 

@@ -642,6 +642,71 @@ def test_overloaded_subvolume_reproduces_periodic_box(oracle_mod, gpu):
     assert per.max() <= PER_PARTICLE_TOL and glob <= 2 * GLOBAL_L2_TOL, (per.max(), glob)
 
 
+# ------------------------------------------- block decomposition with the x2 refinement rule --
+
+def test_accel_blocks_matches_periodic_box_and_refines(oracle_mod, gpu):
+    """srpp_accel_blocks: the node volume split into overlapping x-blocks (active range + passive shell), each evolved
+    as an independent open-faced problem, the active particles reconciled.  For 1, 2, 4 initial blocks and for the
+    adaptively refined plans of repeated calls the result is the periodic-box oracle's for EVERY particle; the work
+    duplicated by the shells (sum of block W / box W) is logged."""
+    torch, binding = gpu
+    ncell = (20, 5, 5)                                      # box 64 x 16 x 16: integer lengths
+    pos, box = workloads.scaled_clustered(120000, ncell, seed=61, frac_halo=0.75, n_halo=1, a_range=(0.6, 0.6))
+    assert box[0] == 64.0
+    n = pos.shape[0]
+    eps = 0.05
+    prm = oracle_mod.make_params(box, 3.0, eps)
+    ref, st = oracle_mod.accel(pos, prm, stats=True)
+    d = torch.from_numpy(pos).cuda()
+    sol = binding.Solver(box, ncell, 3.0, eps, n_max=n)
+    sol.build_mesh(d)
+    sol.accel()
+    w_box = sol.get_stats()["candidate_pairs"]
+    refined = 0
+    for nblocks in (1, 2, 8):
+        sol.blocks_init(nblocks)
+        prev_count = nblocks
+        for call in range(4 if nblocks == 8 else 1):
+            acc, blocks = sol.accel_blocks(d)
+            torch.cuda.synchronize()
+            a = acc.cpu().numpy()
+            assert np.all(a[:, 3] == 0.0)
+            per, glob = oracle_mod.error_norms(a, ref, st["allowance"])
+            # (the shell that wraps through x = L is shifted with one fp32 rounding, DESIGN.md: still inside the bars)
+            assert per.max() <= PER_PARTICLE_TOL and glob <= GLOBAL_L2_TOL, (nblocks, call, per.max(), glob)
+            assert sum(b["n_active"] for b in blocks) == n                       # a partition of the particles
+            assert blocks[0]["x0"] == 0.0 and blocks[-1]["x1"] == box[0]
+            assert all(blocks[i]["x1"] == blocks[i + 1]["x0"] for i in range(len(blocks) - 1))
+            assert len(blocks) >= prev_count                                     # the plan only refines
+            refined = max(refined, max(b["level"] for b in blocks))
+            prev_count = len(blocks)
+            dup = sum(b["candidate_pairs"] for b in blocks) / w_box
+            ms = [b["ms"] for b in blocks]
+            print("blocks: initial %d, call %d: %d blocks, levels %s, duplicated work %.3f, block ms max/mean %.2f, "
+                  "per-particle %.2e, L2 %.2e" % (nblocks, call, len(blocks), [b["level"] for b in blocks], dup,
+                                                  max(ms) / (sum(ms) / len(ms)), per.max(), glob))
+            assert dup >= 0.999
+    assert refined >= 1, "one halo holds 75 % of the particles: its block is > 2x the mean and must have been split"
+    # open parent x axis: blocks see no images across the faces
+    sol.set_boundary((0, 1, 1))
+    sol.blocks_init(3)
+    acc, blocks = sol.accel_blocks(d)
+    ref_o, st_o = oracle_mod.accel(pos, oracle_mod.make_params(box, 3.0, eps, periodic=(0, 1, 1)), stats=True)
+    per, glob = oracle_mod.error_norms(acc.cpu().numpy(), ref_o, st_o["allowance"])
+    assert per.max() <= PER_PARTICLE_TOL and glob <= GLOBAL_L2_TOL, (per.max(), glob)
+    # error paths
+    with pytest.raises(binding.SrppError) as e:
+        sol.blocks_init(0)
+    assert e.value.status == -1
+    sol2 = binding.Solver((19.2, 16.0, 16.0), (6, 5, 5), 3.0, eps, n_max=10)
+    with pytest.raises(binding.SrppError) as e:
+        sol2.blocks_init(2)                                                     # non-integer box length
+    assert e.value.status == -2
+    with pytest.raises(binding.SrppError) as e:
+        sol2.accel_blocks(torch.zeros((4, 4), device="cuda"))                   # no plan
+    assert e.value.status == -5
+
+
 # --------------------------------------------------------------- most bound particle (PAPER.md:93-97) --
 
 def _mbp_check(oracle_mod, gpu, pos, hs, eps):
