@@ -71,6 +71,9 @@ typedef struct {
   uint32_t max_cell_count;  /* largest cell occupancy                                                       */
   uint32_t uniform_mass;    /* 1 if every particle carries the same mass (fast path taken)                   */
   uint64_t kernel_launches; /* CUDA kernels this context has launched since srpp_create (all calls)          */
+  uint64_t rebins_incremental; /* re-bins inside srpp_subcycle done by the incremental merge ...               */
+  uint64_t rebins_full;        /* ... and by a full rebuild (too many movers), since srpp_create                */
+  uint64_t last_movers;        /* particles that changed cell in the last sub-step of the last srpp_subcycle    */
 } srpp_stats;
 
 /* Device times of the last srpp_build_mesh / srpp_accel, from CUDA events the library records on ITS
@@ -79,6 +82,8 @@ typedef struct {
   float mesh_ms;   /* A1-A4: all binning kernels of the last srpp_build_mesh                                */
   float accel_ms;  /* A5-A6: whole srpp_accel (work plan + PP force kernel + write-back)                     */
   float force_ms;  /* A5 only: the PP force kernel launch                                                    */
+  float rebin_ms;  /* mean incremental re-bin of the last srpp_subcycle (movers' sort + merge)                */
+  float kick_stream_ms; /* mean fused kick + stream + mover detection pass of the last srpp_subcycle          */
 } srpp_timings;
 
 /* The six default coefficients (degree-5 fit in s to a Gaussian-filtered point
@@ -215,7 +220,10 @@ int32_t srpp_stream(srpp_ctx* ctx, float* pos_mass, const float* vel, float dt, 
  *   pos_mass, vel   device float4[n], updated in place
  *   acc             device float4[n]: accelerations of the LAST sub-step, caller's order (.w = 0)
  * On return the chaining mesh held by the context is the mesh of the RETURNED positions (srpp_get_mesh, or a following
- * srpp_accel / srpp_subcycle, may use it).  Synchronises the stream (domain check of every re-bin).
+ * srpp_accel, may use it).  Between the first and the last sub-step the state stays in chaining-mesh order: kick and
+ * streams are one coalesced pass over the force kernel's accumulators, and the mesh is repaired by an incremental
+ * re-bin (only the particles that changed cell are sorted and merged back; result bit-identical to a full build), with
+ * a full rebuild as fall-back when more than n/4 particles changed cell.  Synchronises the stream once per sub-step.
  * Errors: INVALID_ARG (null / misaligned pointer, nsub < 0, non-finite dt or kdt), WORKSPACE, DOMAIN, STATE, CUDA. */
 int32_t srpp_subcycle(srpp_ctx* ctx, float* pos_mass, float* vel, float* acc, float dt, float kdt, int32_t nsub,
                       int64_t n);

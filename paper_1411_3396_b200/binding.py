@@ -31,7 +31,8 @@ class SrppParams(C.Structure):
 
 class SrppStats(C.Structure):
     _fields_ = [("work_items", C.c_uint64), ("pair_slots", C.c_uint64), ("candidate_pairs", C.c_uint64),
-                ("max_cell_count", C.c_uint32), ("uniform_mass", C.c_uint32), ("kernel_launches", C.c_uint64)]
+                ("max_cell_count", C.c_uint32), ("uniform_mass", C.c_uint32), ("kernel_launches", C.c_uint64),
+                ("rebins_incremental", C.c_uint64), ("rebins_full", C.c_uint64), ("last_movers", C.c_uint64)]
 
 
 class SrppBlockInfo(C.Structure):
@@ -43,7 +44,8 @@ SRPP_MAX_BLOCKS = 64
 
 
 class SrppTimings(C.Structure):
-    _fields_ = [("mesh_ms", C.c_float), ("accel_ms", C.c_float), ("force_ms", C.c_float)]
+    _fields_ = [("mesh_ms", C.c_float), ("accel_ms", C.c_float), ("force_ms", C.c_float), ("rebin_ms", C.c_float),
+                ("kick_stream_ms", C.c_float)]
 
 
 class SrppError(RuntimeError):

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsrpp.so")
-SOURCES = ["srpp_api.cu", "srpp_mesh.cu", "srpp_force.cu", "srpp_mbp.cu", "srpp_blocks.cu", "srpp_probe.cu"]
+SOURCES = ["srpp_api.cu", "srpp_mesh.cu", "srpp_force.cu", "srpp_mbp.cu", "srpp_blocks.cu", "srpp_subcycle.cu", "srpp_probe.cu"]
 HEADERS = [os.path.join(CSRC, "srpp_internal.cuh"), os.path.join(ROOT, "include", "srpp.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -19,7 +19,7 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
   const size_t o_flags = take(sizeof(DevFlags));
-  const size_t o_v0 = take(4 * nn), o_v1 = take(4 * nn), o_keys = take(4 * nn);
+  const size_t o_v0 = take(4 * nn), o_v1 = take(4 * nn), o_v2 = take(4 * nn), o_keys = take(4 * nn), o_keys1 = take(4 * nn);
   const size_t o_ctl = take(sort_ctl_bytes());
   const size_t o_status = take(8 * (size_t)kSortMaxBins * (nn / kPassTile + 1));   // [tiles][bins] look-back words
   const size_t o_cs = take(4 * (ncells + 1));
@@ -27,11 +27,36 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   const size_t o_prefix = take(8 * (ncells + 1));
   const size_t o_tmp = take(8 * ((ncells + 4095) / 4096 + 1));
   const size_t o_acc = take(8 * 3 * nn);
+  // sorted-space state of srpp_subcycle and the incremental re-bin
+  const size_t o_sorted1 = take(16 * nn), o_vs0 = take(16 * nn), o_vs1 = take(16 * nn);
+  const size_t o_pf = take(4 * (nn + 1)), o_mmask = take(4 * (nn / 32 + 2)), o_mwp = take(8 * (nn / 32 + 2));
+  const size_t o_tm = take(8 * (nn / 1024 + 2)), o_stmp = take(8 * (nn / 32 / 4096 + nn / 1024 / 4096 + 8));
+  const size_t mcap = nn / 4 + 1024;
+  const size_t o_ms = take(4 * mcap), o_msr = take(4 * mcap), o_mpos = take(16 * mcap), o_mis = take(4 * mcap), o_mss = take(4 * mcap);
+  const size_t o_mflags = take(sizeof(DevFlags)), o_mctl = take(sort_ctl_bytes());
+  const size_t o_mstatus = take(8 * (size_t)kSortMaxBins * (mcap / kPassTile + 1));
+  const size_t o_msorted = take(16 * mcap), o_mtmp = take(16 * mcap), o_mv0 = take(4 * mcap), o_mv1 = take(4 * mcap);
+  const size_t o_mkeys = take(4 * mcap), o_mcs = take(4 * (ncells + 1));
   if (c) {
     char* b = c->ws;
     c->flags = (DevFlags*)(b + o_flags);
     c->vals[0] = (uint32_t*)(b + o_v0); c->vals[1] = (uint32_t*)(b + o_v1);
-    c->sorted_keys_buf = (uint32_t*)(b + o_keys);
+    c->vals_alt = (uint32_t*)(b + o_v2);
+    c->keys_buf[0] = (uint32_t*)(b + o_keys); c->keys_buf[1] = (uint32_t*)(b + o_keys1);
+    c->sorted_buf[0] = (float4*)(b + o_sorted); c->sorted_buf[1] = (float4*)(b + o_sorted1);
+    c->vel_s[0] = (float4*)(b + o_vs0); c->vel_s[1] = (float4*)(b + o_vs1);
+    c->prefix_f = (uint32_t*)(b + o_pf); c->mover_mask = (uint32_t*)(b + o_mmask);
+    c->mover_wprefix = (unsigned long long*)(b + o_mwp); c->tile_movers = (unsigned long long*)(b + o_tm);
+    c->sub_scan_tmp = (unsigned long long*)(b + o_stmp);
+    c->mover_slots = (uint32_t*)(b + o_ms); c->mover_slot_by_rank = (uint32_t*)(b + o_msr);
+    c->mover_pos = (float4*)(b + o_mpos); c->mover_idx_sorted = (uint32_t*)(b + o_mis); c->mover_slot_sorted = (uint32_t*)(b + o_mss);
+    c->m_flags = (DevFlags*)(b + o_mflags); c->m_ctl = (uint32_t*)(b + o_mctl);
+    if (c->m_status != (unsigned long long*)(b + o_mstatus)) c->status_n_movers = 0;
+    c->m_status = (unsigned long long*)(b + o_mstatus);
+    c->m_sorted = (float4*)(b + o_msorted); c->m_tmp = (float4*)(b + o_mtmp);
+    c->m_vals[0] = (uint32_t*)(b + o_mv0); c->m_vals[1] = (uint32_t*)(b + o_mv1);
+    c->m_keys = (uint32_t*)(b + o_mkeys); c->m_cell_start = (uint32_t*)(b + o_mcs);
+    c->m_cap = (int64_t)mcap;
     c->sort_ctl = (uint32_t*)(b + o_ctl);
     if (c->sort_status != (unsigned long long*)(b + o_status)) c->status_n = 0;   // the array moved: clear before use
     c->sort_status = (unsigned long long*)(b + o_status);
@@ -199,6 +224,8 @@ void srpp_destroy(srpp_ctx* c) {
   if (!c) return;
   for (int i = 0; i < kNumEvents; ++i)
     if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+  for (int i = 0; i < 2; ++i)
+    if (c->ev_sub[i]) cudaEventDestroy(c->ev_sub[i]);
   free_block_plan(c);
   delete c;
 }
@@ -220,6 +247,8 @@ int32_t srpp_set_timing(srpp_ctx* c, int32_t enable) {
 int32_t srpp_get_timings(srpp_ctx* c, srpp_timings* t) {
   if (!c || !t) return SRPP_ERR_INVALID_ARG;
   t->mesh_ms = t->accel_ms = t->force_ms = -1.0f;
+  t->rebin_ms = c->rebin_count ? c->rebin_ms_sum / (float)c->rebin_count : -1.0f;
+  t->kick_stream_ms = c->rebin_count ? c->subkick_ms_sum / (float)c->rebin_count : -1.0f;
   if (!c->timing) return SRPP_ERR_STATE;
   cudaError_t e = cudaStreamSynchronize(c->stream);
   if (e == cudaSuccess && c->ev_mesh_valid) e = cudaEventElapsedTime(&t->mesh_ms, c->ev[kEvMesh0], c->ev[kEvMesh1]);
@@ -342,6 +371,9 @@ int32_t srpp_get_stats(srpp_ctx* c, srpp_stats* s) {
   s->max_cell_count = c->flags_host.max_cell_count;
   s->uniform_mass = c->uniform_mass ? 1u : 0u;
   s->kernel_launches = c->launches;
+  s->rebins_incremental = c->rebin_incremental;
+  s->rebins_full = c->rebin_full;
+  s->last_movers = c->last_movers;
   return SRPP_OK;
 }
 
@@ -357,24 +389,6 @@ int32_t srpp_stream(srpp_ctx* c, float* pos_mass, const float* vel, float dt, in
   if (const int32_t d = check_device(c)) return d;
   const cudaError_t e = launch_stream(c, (float4*)pos_mass, (const float4*)vel, dt, n);
   return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
-}
-
-int32_t srpp_subcycle(srpp_ctx* c, float* pos_mass, float* vel, float* acc, float dt, float kdt, int32_t nsub, int64_t n) {
-  if (!c || n < 0 || n >= ((int64_t)1 << 31) || nsub < 0 || !isfinite(dt) || !isfinite(kdt) ||
-      (n > 0 && (!pos_mass || !vel || !acc)) || misaligned16(pos_mass) || misaligned16(vel) || misaligned16(acc))
-    return SRPP_ERR_INVALID_ARG;
-  if (const int32_t d = check_device(c)) return d;
-  const float half = 0.5f * dt;            // exact in fp32
-  int32_t rc = SRPP_OK;
-  for (int32_t s = 0; s < nsub; ++s) {
-    if ((rc = srpp_stream(c, pos_mass, vel, half, n)) != SRPP_OK) return rc;
-    if ((rc = srpp_build_mesh(c, pos_mass, n)) != SRPP_OK) return rc;
-    if ((rc = srpp_accel(c, acc)) != SRPP_OK) return rc;
-    if ((rc = srpp_kick(c, vel, acc, kdt, n)) != SRPP_OK) return rc;
-    if ((rc = srpp_stream(c, pos_mass, vel, half, n)) != SRPP_OK) return rc;
-  }
-  // the context's mesh is the mesh of the returned positions
-  return srpp_build_mesh(c, pos_mass, n);
 }
 
 int32_t srpp_step_host(srpp_ctx* c, const float* pos_mass_host, float* vel_host, float* acc_host, float kdt,

@@ -434,13 +434,6 @@ __global__ void __launch_bounds__(256) k_kick(float4* __restrict__ vel, const fl
   }
 }
 
-__device__ __forceinline__ float wrap_coord(float y, float L) {
-  if (y >= L) y -= L;
-  else if (y < 0.f) y += L;
-  if (!(y < L)) y = 0.f;
-  return y;
-}
-
 __global__ void __launch_bounds__(256) k_stream(float4* __restrict__ pos, const float4* __restrict__ vel, float dt,
                                                  float Lx, float Ly, float Lz, int64_t n) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
@@ -471,13 +464,12 @@ cudaError_t launch_scan_u64(cudaStream_t st, unsigned long long* data, int n, un
   return cudaGetLastError();
 }
 
-cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
+cudaError_t launch_accel_sorted(srpp_ctx* c) {
   cudaStream_t st = c->stream;
   const int64_t n = c->n;
   const int32_t ncells = c->geo.ncells;
   cudaError_t e;
   if (n == 0) return cudaSuccess;
-  if (c->timing) cudaEventRecord(c->ev[kEvAccel0], st);
   // reset queue head + statistics (keep the binning flags)
   if ((e = cudaMemsetAsync(&c->flags->max_cell_count, 0, sizeof(DevFlags) - offsetof(DevFlags, max_cell_count), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(c->acc64, 0, sizeof(double) * 3 * (size_t)n, st)) != cudaSuccess) return e;
@@ -491,12 +483,27 @@ cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
   else
     k_pp_force<false><<<grid, kForceThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
   if (c->timing) cudaEventRecord(c->ev[kEvForce1], st);
-  const int grid_ew = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
-  const int grid_wb = (int)std::min<int64_t>((n + 1023) / 1024, (int64_t)c->num_sms * 16);
-  k_write_back<<<grid_wb, 256, 0, st>>>(c->acc64, c->perm, n, c->uniform_mass ? c->mass0 : 1.0f, acc);
-  c->launches += 6;
-  if (c->timing) { cudaEventRecord(c->ev[kEvAccel1], st); c->ev_accel_valid = true; }
+  c->launches += 5;
   return cudaGetLastError();
+}
+
+cudaError_t launch_write_back(srpp_ctx* c, float4* acc) {
+  const int64_t n = c->n;
+  if (n == 0) return cudaSuccess;
+  const int grid_wb = (int)std::min<int64_t>((n + 1023) / 1024, (int64_t)c->num_sms * 16);
+  k_write_back<<<grid_wb, 256, 0, c->stream>>>(c->acc64, c->perm, n, c->uniform_mass ? c->mass0 : 1.0f, acc);
+  c->launches += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_accel(srpp_ctx* c, float4* acc) {
+  cudaStream_t st = c->stream;
+  if (c->n == 0) return cudaSuccess;
+  if (c->timing) cudaEventRecord(c->ev[kEvAccel0], st);
+  cudaError_t e = launch_accel_sorted(c);
+  if (e == cudaSuccess) e = launch_write_back(c, acc);
+  if (c->timing) { cudaEventRecord(c->ev[kEvAccel1], st); c->ev_accel_valid = true; }
+  return e;
 }
 
 cudaError_t launch_kick(srpp_ctx* c, float4* vel, const float4* acc, float kdt, int64_t n) {

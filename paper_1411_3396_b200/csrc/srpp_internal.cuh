@@ -64,6 +64,32 @@ struct ForceConst {
   int32_t fine_items;    // tiny problem: 16-target items so that every resident warp gets work
 };
 
+#ifdef __CUDACC__
+// A1 (R10, R11): one IEEE multiply per axis (never contracted: there is nothing to fuse with), floor, clamp.
+__device__ __forceinline__ uint32_t cell_key(const float4& p, const Geometry& g) {
+  int cx = (int)floorf(__fmul_rn(p.x, g.inv_cell[0]));
+  int cy = (int)floorf(__fmul_rn(p.y, g.inv_cell[1]));
+  int cz = (int)floorf(__fmul_rn(p.z, g.inv_cell[2]));
+  cx = max(min(cx, g.ncell[0] - 1), 0);       // the lower clamp only matters for inputs that already raised DOMAIN
+  cy = max(min(cy, g.ncell[1] - 1), 0);
+  cz = max(min(cz, g.ncell[2] - 1), 0);
+  return (uint32_t)cx + (uint32_t)g.ncell[0] * ((uint32_t)cy + (uint32_t)g.ncell[1] * (uint32_t)cz);
+}
+
+__device__ __forceinline__ bool in_domain(const float4& p, const Geometry& g) {
+  return (p.x >= 0.f) && (p.x < g.box[0]) && (p.y >= 0.f) && (p.y < g.box[1]) && (p.z >= 0.f) && (p.z < g.box[2]);
+}
+
+// stream wrap (R13, R17): one box length at most; a value that rounds to L becomes 0
+__device__ __forceinline__ float wrap_coord(float y, float L) {
+  if (y >= L) y -= L;
+  else if (y < 0.f) y += L;
+  if (!(y < L)) y = 0.f;
+  return y;
+}
+
+#endif
+
 }  // namespace srpp
 
 struct srpp_ctx {
@@ -88,14 +114,35 @@ struct srpp_ctx {
   size_t ws_bytes;
   srpp::DevFlags* flags;
   uint32_t* vals[2];         // original indices, ping-pong (unequal masses) / perm of the last pass
-  uint32_t* sorted_keys_buf; // cell ids in sorted order, written by the last pass
+  uint32_t* vals_alt;        // third index buffer: the incremental re-bin writes the new perm beside the current one
+  uint32_t* keys_buf[2];     // cell ids in sorted order: [0] written by a full build, [1] its ping-pong partner
+  float4* sorted_buf[2];     // sorted positions: [0] written by a full build, [1] ping-pong partner of the re-bin
+  float4* vel_s[2];          // velocities in sorted order (srpp_subcycle), ping-pong
+  uint32_t* prefix_f;        // [n+1] exclusive prefix of the mover flags over the sorted slots
+  uint32_t* mover_mask;      // [n/32+1] bit i set: particle with original index i changed cell
+  unsigned long long* mover_wprefix;  // [n/32+2] exclusive prefix of popc(mover_mask)
+  unsigned long long* tile_movers;    // [n/1024+2] movers per 1024 sorted slots, scanned in place
+  unsigned long long* sub_scan_tmp;   // scan scratch
+  uint32_t* mover_slots;     // [m_cap] unordered list of the sorted slots that hold movers
+  uint32_t* mover_slot_by_rank;  // [m_cap] slot of the j-th mover in ascending original index
+  float4* mover_pos;         // [m_cap] their new positions (input of the movers' sort)
+  uint32_t* mover_idx_sorted;    // [m_cap] original index, in (new cell, index) order
+  uint32_t* mover_slot_sorted;   // [m_cap] old slot, same order
+  // second sort buffer set (the movers)
+  srpp::DevFlags* m_flags; uint32_t* m_ctl; unsigned long long* m_status; float4* m_sorted; float4* m_tmp;
+  uint32_t* m_vals[2]; uint32_t* m_keys; uint32_t* m_cell_start;
+  int64_t status_n_movers;
+  int64_t m_cap;             // movers the second set is sized for (n/4): beyond it the re-bin falls back to a full build
+  uint64_t rebin_incremental, rebin_full, last_movers;   // counters (srpp_get_stats)
+  cudaEvent_t ev_sub[2];     // timing of the re-bins inside srpp_subcycle
+  float rebin_ms_sum, subkick_ms_sum; int rebin_count;
   uint32_t* sort_ctl;        // tile tickets + global digit histograms (cleared by every build)
   unsigned long long* sort_status;  // [tiles][kSortMaxBins] look-back status words, epoch-tagged
   int64_t status_n;          // n the status array was last cleared for (0 = never)
   uint32_t sort_epoch;       // tag of the last pass launched
   float4* pos_tmp;           // payload ping-pong buffer (aliases acc64: mesh build and accel never overlap)
   uint32_t* cell_start;      // [ncells+1]
-  float4* sorted;            // [n]
+  float4* sorted;            // [n] current sorted positions (== sorted_buf[0] after a full build)
   unsigned long long* item_prefix;  // [ncells+1] exclusive prefix of per-cell work items
   unsigned long long* scan_tmp;     // block sums for the 64-bit scan
   double* acc64;             // [3n] fp64 accumulators, sorted order
@@ -114,13 +161,26 @@ struct srpp_ctx {
 
 namespace srpp {
 
+// buffer set of one sort_by_cell call
+struct SortBufs {
+  DevFlags* flags; uint32_t* ctl; unsigned long long* status; int64_t* status_n;
+  float4* out_sorted; float4* tmp_pos; uint32_t* vals[2]; uint32_t* keys_out; uint32_t* cell_start;
+  uint32_t* perm;            // result: == vals[(passes - 1) & 1]
+};
+
 size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* ctx /*nullable: fill pointers*/);
 
 // srpp_mesh.cu
 cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n);
+cudaError_t sort_by_cell(srpp_ctx* c, SortBufs& sb, const float4* pos_mass, int64_t n);
 void plan_sort(int32_t ncells, int* passes, int* digit_bits);
 // srpp_force.cu
-cudaError_t launch_accel(srpp_ctx* c, float4* acc);
+cudaError_t launch_accel(srpp_ctx* c, float4* acc);            // force + write-back
+cudaError_t launch_accel_sorted(srpp_ctx* c);                  // force only: fp64 accumulators in sorted order
+cudaError_t launch_write_back(srpp_ctx* c, float4* acc);       // A6
+// srpp_subcycle.cu
+cudaError_t launch_subcycle(srpp_ctx* c, float4* pos_mass, float4* vel, float4* acc, float dt, float kdt, int nsub,
+                            int64_t n, int32_t* status_out);
 cudaError_t launch_kick(srpp_ctx* c, float4* vel, const float4* acc, float kdt, int64_t n);
 cudaError_t launch_stream(srpp_ctx* c, float4* pos_mass, const float4* vel, float dt, int64_t n);
 int query_force_occupancy();

@@ -35,21 +35,6 @@
 namespace srpp {
 
 // ------------------------------------------------------------------------------ small helpers --
-// A1 (R10, R11): one IEEE multiply per axis (never contracted: there is nothing to fuse with), floor, clamp.
-__device__ __forceinline__ uint32_t cell_key(const float4& p, const Geometry& g) {
-  int cx = (int)floorf(__fmul_rn(p.x, g.inv_cell[0]));
-  int cy = (int)floorf(__fmul_rn(p.y, g.inv_cell[1]));
-  int cz = (int)floorf(__fmul_rn(p.z, g.inv_cell[2]));
-  cx = max(min(cx, g.ncell[0] - 1), 0);       // the lower clamp only matters for inputs that already raised DOMAIN
-  cy = max(min(cy, g.ncell[1] - 1), 0);
-  cz = max(min(cz, g.ncell[2] - 1), 0);
-  return (uint32_t)cx + (uint32_t)g.ncell[0] * ((uint32_t)cy + (uint32_t)g.ncell[1] * (uint32_t)cz);
-}
-
-__device__ __forceinline__ bool in_domain(const float4& p, const Geometry& g) {
-  return (p.x >= 0.f) && (p.x < g.box[0]) && (p.y >= 0.f) && (p.y < g.box[1]) && (p.z >= 0.f) && (p.z < g.box[2]);
-}
-
 // Exclusive scan of one value per thread over a kThreads-wide CTA; `scratch` holds 32 words.
 template <int kThreads>
 __device__ __forceinline__ uint32_t cta_exclusive_scan(uint32_t v, uint32_t* scratch) {
@@ -417,19 +402,19 @@ void plan_sort(int32_t ncells, int* passes, int* digit_bits) {
   *digit_bits = (bits + p - 1) / p;
 }
 
-cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n) {
+// Stable sort of n particles by cell id into the buffers of `sb` (the context's own for srpp_build_mesh, a second set
+// for the movers of the incremental re-bin): sb.out_sorted / sb.perm / sb.keys_out / sb.cell_start.
+cudaError_t sort_by_cell(srpp_ctx* c, SortBufs& sb, const float4* pos_mass, int64_t n) {
   cudaStream_t st = c->stream;
   cudaError_t e;
-  // flag block + sort control block (tickets, digit histograms) are contiguous: one memset
-  if ((e = cudaMemsetAsync(c->flags, 0, sizeof(DevFlags), st)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(c->sort_ctl, 0, sort_ctl_bytes(), st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(sb.flags, 0, sizeof(DevFlags), st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(sb.ctl, 0, sort_ctl_bytes(), st)) != cudaSuccess) return e;
   const int32_t ncells = c->geo.ncells;
   const int passes = c->sort_passes, dbits = c->sort_digit_bits, nbins = 1 << dbits;
-  // the last pass writes into sorted / vals[f]; earlier passes alternate with the scratch set
+  // the last pass writes into out_sorted / vals[f]; earlier passes alternate with the scratch set
   const int f = (passes - 1) & 1;
-  c->perm = c->vals[f];
-  if (n == 0) return cudaMemsetAsync(c->cell_start, 0, sizeof(uint32_t) * ((size_t)ncells + 1), st);
-  if (c->timing) cudaEventRecord(c->ev[kEvMesh0], st);
+  sb.perm = sb.vals[f];
+  if (n == 0) return cudaMemsetAsync(sb.cell_start, 0, sizeof(uint32_t) * ((size_t)ncells + 1), st);
 
   const size_t smem_packed = sort_pass_smem(nbins, true), smem_plain = sort_pass_smem(nbins, false);
   if (!c->sort_attr_set) {
@@ -438,24 +423,22 @@ cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n) {
     c->sort_attr_set = true;
   }
   const int64_t tiles = (n + kSortTile - 1) / kSortTile, ptiles = (n + kPassTile - 1) / kPassTile;
-  // the look-back status words are tagged with an epoch, so they are cleared only when the array moves or the
-  // epoch counter wraps (tags of another layout / an earlier life of the workspace must not be mistaken for ours)
-  if (c->status_n != n || c->sort_epoch > 0x3ffffff0u) {
-    if ((e = cudaMemsetAsync(c->sort_status, 0, sizeof(unsigned long long) * (size_t)ptiles * kSortMaxBins, st)) != cudaSuccess) return e;
-    c->status_n = n;
-    c->sort_epoch = 0;
+  // the look-back status words are tagged with an epoch, so they are cleared only when the array moves, grows, or
+  // the epoch counter wraps (tags of another layout / an earlier life of the workspace must not be mistaken for ours)
+  if (c->sort_epoch > 0x3ffffff0u) { c->sort_epoch = 0; c->status_n = 0; c->status_n_movers = 0; }
+  if (*sb.status_n < n || *sb.status_n == 0) {
+    if ((e = cudaMemsetAsync(sb.status, 0, sizeof(unsigned long long) * (size_t)ptiles * kSortMaxBins, st)) != cudaSuccess) return e;
+    *sb.status_n = n;
   }
   const int blocks = (int)std::min<int64_t>(ptiles, (int64_t)c->num_sms * kPassCtasPerSm);
   const int hblocks = (int)std::min<int64_t>(tiles, (int64_t)c->num_sms * 2);
-  c->sort_blocks = blocks;
 
-  uint32_t* tickets = c->sort_ctl;
-  uint32_t* ghist = c->sort_ctl + 64;
-  // payload buffers: set f = {sorted, vals[f]}, set f^1 = {pos_tmp, vals[f^1]}
+  uint32_t* tickets = sb.ctl;
+  uint32_t* ghist = sb.ctl + 64;
   float4* posbuf[2];
-  posbuf[f] = c->sorted;
-  posbuf[f ^ 1] = c->pos_tmp;
-  k_sort_prepass<<<hblocks, kSortThreads, 0, st>>>(pos_mass, n, c->geo, c->flags, passes, dbits, ghist);
+  posbuf[f] = sb.out_sorted;
+  posbuf[f ^ 1] = sb.tmp_pos;
+  k_sort_prepass<<<hblocks, kSortThreads, 0, st>>>(pos_mass, n, c->geo, sb.flags, passes, dbits, ghist);
   const float4* pin = pos_mass;
   const uint32_t* iin = nullptr;
   for (int p = 0; p < passes; ++p) {
@@ -463,15 +446,30 @@ cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n) {
     const int o = p & 1;
     const int first = p == 0, last = p == passes - 1;
     const uint32_t epoch = ++c->sort_epoch;
-    k_sort_pass<true><<<blocks, kPassThreads, smem_packed, st>>>(pin, iin, posbuf[o], c->vals[o], c->sorted_keys_buf, pos_mass, n, c->geo, shift, nbins, first, last, ghist + (size_t)p * kSortMaxBins, c->sort_status, tickets + p, epoch, c->flags);
-    k_sort_pass<false><<<blocks, kPassThreads, smem_plain, st>>>(pin, iin, posbuf[o], c->vals[o], c->sorted_keys_buf, pos_mass, n, c->geo, shift, nbins, first, last, ghist + (size_t)p * kSortMaxBins, c->sort_status, tickets + p, epoch, c->flags);
-    pin = posbuf[o]; iin = c->vals[o];
+    k_sort_pass<true><<<blocks, kPassThreads, smem_packed, st>>>(pin, iin, posbuf[o], sb.vals[o], sb.keys_out, pos_mass, n, c->geo, shift, nbins, first, last, ghist + (size_t)p * kSortMaxBins, sb.status, tickets + p, epoch, sb.flags);
+    k_sort_pass<false><<<blocks, kPassThreads, smem_plain, st>>>(pin, iin, posbuf[o], sb.vals[o], sb.keys_out, pos_mass, n, c->geo, shift, nbins, first, last, ghist + (size_t)p * kSortMaxBins, sb.status, tickets + p, epoch, sb.flags);
+    pin = posbuf[o]; iin = sb.vals[o];
   }
-  c->sorted_keys = c->sorted_keys_buf;
   const int grid_ew = (int)((n + 2047) / 2048);     // one trip per thread: the loads of all CTAs overlap
-  k_cell_start<<<grid_ew, 256, 0, st>>>(c->sorted_keys, n, ncells, c->cell_start);
+  k_cell_start<<<grid_ew, 256, 0, st>>>(sb.keys_out, n, ncells, sb.cell_start);
   c->launches += 2 + 2 * (uint64_t)passes;
-  if (c->timing) { cudaEventRecord(c->ev[kEvMesh1], st); c->ev_mesh_valid = true; }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n) {
+  cudaStream_t st = c->stream;
+  if (c->timing && n > 0) cudaEventRecord(c->ev[kEvMesh0], st);
+  // a full build always lands in the primary buffers (the incremental re-bin of srpp_subcycle ping-pongs)
+  SortBufs sb;
+  sb.flags = c->flags; sb.ctl = c->sort_ctl; sb.status = c->sort_status; sb.status_n = &c->status_n;
+  sb.out_sorted = c->sorted_buf[0]; sb.tmp_pos = c->pos_tmp; sb.vals[0] = c->vals[0]; sb.vals[1] = c->vals[1];
+  sb.keys_out = c->keys_buf[0]; sb.cell_start = c->cell_start; sb.perm = nullptr;
+  const cudaError_t e = sort_by_cell(c, sb, pos_mass, n);
+  if (e != cudaSuccess) return e;
+  c->sorted = c->sorted_buf[0];
+  c->sorted_keys = c->keys_buf[0];
+  c->perm = sb.perm;
+  if (c->timing && n > 0) { cudaEventRecord(c->ev[kEvMesh1], st); c->ev_mesh_valid = true; }
   return cudaGetLastError();
 }
 

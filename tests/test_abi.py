@@ -30,8 +30,9 @@ def test_header_symbols_exported(lib):
 
 def test_struct_layout_matches_header():
     assert C.sizeof(binding.SrppParams) == 3 * 4 + 3 * 4 + 4 + 4 + 6 * 4
-    assert C.sizeof(binding.SrppStats) == 8 * 3 + 4 * 2 + 8
-    assert C.sizeof(binding.SrppTimings) == 12
+    assert C.sizeof(binding.SrppStats) == 8 * 3 + 4 * 2 + 8 + 8 * 3
+    assert C.sizeof(binding.SrppTimings) == 20
+    assert C.sizeof(binding.SrppBlockInfo) == 48
 
 
 def test_default_poly_bits():

@@ -417,10 +417,57 @@ def test_subcycle_several_substeps_vs_oracle(oracle_mod, gpu):
     assert np.abs(d).max() <= 2e-5
     per, glob = oracle_mod.error_norms(a, ao)
     assert glob <= 1e-4          # accelerations at slightly different positions (the differences above)
+    # the mesh after four chained incremental re-bins is the oracle's mesh of the returned positions, bit for bit
+    st = sol.get_stats()
+    assert st["rebins_incremental"] == 4 and st["rebins_full"] == 0, st
+    cs, perm, srt = (t.cpu().numpy() for t in sol.get_mesh())
+    o_cs, o_perm, o_srt = oracle_mod.build_mesh(x, box, ncell)
+    assert np.array_equal(cs.view(np.uint32), o_cs) and np.array_equal(perm.view(np.uint32), o_perm)
+    assert np.array_equal(srt.view(np.uint32), o_srt.view(np.uint32))
     # nsub = 0: nothing moves, the mesh is (re)built
     x_before = d_pos.clone()
     sol.subcycle(d_pos, d_vel, dt, dt, 0)
     assert torch.equal(x_before, d_pos)
+
+
+@pytest.mark.parametrize("masses", [False, True])
+def test_subcycle_rebin_paths_bit_exact(oracle_mod, gpu, masses):
+    """The incremental re-bin against orc_build_mesh after EVERY sub-step, for small and large mover fractions (the
+    latter takes the full-rebuild fall-back), equal and unequal masses, heavy cells, and a step in which nobody moves."""
+    torch, binding = gpu
+    ncell = (7, 6, 5)
+    pos, box = workloads.scaled_clustered(150000, ncell, seed=71, frac_halo=0.7, n_halo=6, a_range=(0.2, 1.0))
+    rng = np.random.default_rng(71)
+    n = pos.shape[0]
+    if masses:
+        pos[:, 3] = rng.uniform(0.5, 2.0, n).astype(np.float32)
+    vel = np.zeros_like(pos)
+    vel[:, :3] = rng.normal(0, 1.0, (n, 3)).astype(np.float32)
+    sol = binding.Solver(box, ncell, 3.0, 0.1, n_max=n)
+    d_pos, d_vel = torch.from_numpy(pos.copy()).cuda(), torch.from_numpy(vel.copy()).cuda()
+    x_prev = pos
+    for dt, expect in ((0.0, "none"), (0.05, "incremental"), (0.2, "incremental"), (3.0, "full"), (0.02, "incremental")):
+        before = sol.get_stats() if sol.n >= 0 else {"rebins_incremental": 0, "rebins_full": 0}
+        sol.subcycle(d_pos, d_vel, dt, 0.0, 1)                  # kdt = 0: velocities stay put, dt sets the mover fraction
+        torch.cuda.synchronize()
+        x = d_pos.cpu().numpy()
+        st = sol.get_stats()
+        moved = float(np.mean(oracle_mod.cell_ids(x_prev, box, ncell) != oracle_mod.cell_ids(x, box, ncell)))
+        print("dt %.2f: %.1f %% changed cell (%d movers in the last pass), incremental %d, full %d"
+              % (dt, 100 * moved, st["last_movers"], st["rebins_incremental"], st["rebins_full"]))
+        if expect == "incremental":
+            assert st["rebins_incremental"] == before["rebins_incremental"] + 1 and st["rebins_full"] == before["rebins_full"]
+        elif expect == "full":
+            assert st["rebins_full"] == before["rebins_full"] + 1 and moved > 0.25
+        else:
+            assert st["last_movers"] == 0 and np.array_equal(x, x_prev)
+        cs, perm, srt = (t.cpu().numpy() for t in sol.get_mesh())
+        o_cs, o_perm, o_srt = oracle_mod.build_mesh(x, box, ncell)
+        assert np.array_equal(cs.view(np.uint32), o_cs), dt
+        assert np.array_equal(perm.view(np.uint32), o_perm), dt
+        assert np.array_equal(srt.view(np.uint32), o_srt.view(np.uint32)), dt
+        assert np.array_equal(d_vel.cpu().numpy(), vel)
+        x_prev = x
 
 
 def test_subcycle_active_box_streams_passive_particles(oracle_mod, gpu):
