@@ -19,7 +19,7 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
   const size_t o_flags = take(sizeof(DevFlags));
-  const size_t o_v0 = take(4 * nn), o_v1 = take(4 * nn), o_v2 = take(4 * nn), o_keys = take(4 * nn), o_keys1 = take(4 * nn);
+  const size_t o_v0 = take(4 * nn), o_v1 = take(4 * nn), o_v2 = take(4 * nn), o_keys = take(4 * nn);
   const size_t o_ctl = take(sort_ctl_bytes());
   const size_t o_status = take(8 * (size_t)kSortMaxBins * (nn / kPassTile + 1));   // [tiles][bins] look-back words
   const size_t o_cs = take(4 * (ncells + 1));
@@ -29,7 +29,7 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   const size_t o_acc = take(8 * 3 * nn);
   // sorted-space state of srpp_subcycle and the incremental re-bin
   const size_t o_sorted1 = take(16 * nn), o_vs0 = take(16 * nn), o_vs1 = take(16 * nn);
-  const size_t o_pf = take(4 * (nn + 1)), o_mmask = take(4 * (nn / 32 + 2)), o_mwp = take(8 * (nn / 32 + 2));
+  const size_t o_pf = take(4 * (nn / 32 + 2)), o_fw = take(4 * (nn / 32 + 2)), o_mmask = take(4 * (nn / 32 + 2)), o_mwp = take(8 * (nn / 32 + 2));
   const size_t o_tm = take(8 * (nn / 1024 + 2)), o_stmp = take(8 * (nn / 32 / 4096 + nn / 1024 / 4096 + 8));
   const size_t mcap = nn / 4 + 1024;
   const size_t o_ms = take(4 * mcap), o_msr = take(4 * mcap), o_mpos = take(16 * mcap), o_mis = take(4 * mcap), o_mss = take(4 * mcap);
@@ -42,10 +42,10 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
     c->flags = (DevFlags*)(b + o_flags);
     c->vals[0] = (uint32_t*)(b + o_v0); c->vals[1] = (uint32_t*)(b + o_v1);
     c->vals_alt = (uint32_t*)(b + o_v2);
-    c->keys_buf[0] = (uint32_t*)(b + o_keys); c->keys_buf[1] = (uint32_t*)(b + o_keys1);
+    c->keys_buf[0] = (uint32_t*)(b + o_keys); c->keys_buf[1] = nullptr;
     c->sorted_buf[0] = (float4*)(b + o_sorted); c->sorted_buf[1] = (float4*)(b + o_sorted1);
     c->vel_s[0] = (float4*)(b + o_vs0); c->vel_s[1] = (float4*)(b + o_vs1);
-    c->prefix_f = (uint32_t*)(b + o_pf); c->mover_mask = (uint32_t*)(b + o_mmask);
+    c->prefix_f = (uint32_t*)(b + o_pf); c->flag_words = (uint32_t*)(b + o_fw); c->mover_mask = (uint32_t*)(b + o_mmask);
     c->mover_wprefix = (unsigned long long*)(b + o_mwp); c->tile_movers = (unsigned long long*)(b + o_tm);
     c->sub_scan_tmp = (unsigned long long*)(b + o_stmp);
     c->mover_slots = (uint32_t*)(b + o_ms); c->mover_slot_by_rank = (uint32_t*)(b + o_msr);

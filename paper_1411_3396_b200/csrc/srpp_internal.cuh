@@ -118,7 +118,8 @@ struct srpp_ctx {
   uint32_t* keys_buf[2];     // cell ids in sorted order: [0] written by a full build, [1] its ping-pong partner
   float4* sorted_buf[2];     // sorted positions: [0] written by a full build, [1] ping-pong partner of the re-bin
   float4* vel_s[2];          // velocities in sorted order (srpp_subcycle), ping-pong
-  uint32_t* prefix_f;        // [n+1] exclusive prefix of the mover flags over the sorted slots
+  uint32_t* prefix_f;        // [n/32+2] movers in the slots before each 32-slot flag word
+  uint32_t* flag_words;      // [n/32+2] bit k&31 of word k>>5: the particle in sorted slot k changed cell
   uint32_t* mover_mask;      // [n/32+1] bit i set: particle with original index i changed cell
   unsigned long long* mover_wprefix;  // [n/32+2] exclusive prefix of popc(mover_mask)
   unsigned long long* tile_movers;    // [n/1024+2] movers per 1024 sorted slots, scanned in place
