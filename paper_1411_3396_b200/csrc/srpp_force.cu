@@ -66,14 +66,17 @@ __device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint
 
 // Targets of one work item.  Large cells: 32 lanes x 4 targets (two packed pairs per lane), several items per cell.
 // Cells of <= 48 particles (the uniform background: ~33 per cell) would leave half of a 64-target tile empty, so
-// there the warp is split 4 ways over the SOURCES: 8 lanes x 2 targets = 16 targets per packed pair, 1-3 packed
-// pairs per lane cover the WHOLE cell in one item (the staged sources are shared by all its targets), lane group
-// g = lane / 8 takes sources g, g+4, g+8, ... of the staged tile, and the four partial sums are added with shuffles
-// at the end.  Cells of 49..64 particles take one 64-target item.
-constexpr int kSplit = 4;                       // source phases of the small-cell path
+// there the warp is split over the SOURCES: with S source phases, 32/S lanes x 2 targets = 64/S targets per packed
+// pair, TP packed pairs per lane cover the WHOLE cell in one item (the staged sources are shared by all its targets),
+// lane group g = lane / (32/S) takes sources g, g+S, g+2S, ... of the staged tile, and the S partial sums are added
+// with shuffles at the end.  Cells of <= 40 particles use S = 8 (targets padded to a multiple of 8: 1.10 pair slots
+// per candidate pair at ~33 per cell; S = 4 with its multiples of 16 gave 1.23), 41..48 use S = 4 (48 slots), 49..64
+// take one 64-target item.
+constexpr uint32_t kSplit8MaxCell = 40;         // <= 5 packed pairs of 8 targets
 constexpr uint32_t kSplitMaxCell = 48;          // <= 3 packed pairs of 16 targets
 __device__ __forceinline__ uint32_t targets_per_item(uint32_t n_c, int fine) {
-  if (n_c <= kSplitMaxCell) return fine ? 16u : ((n_c + 15u) / 16u) * 16u;   // fine: tiny problems need more items
+  if (n_c <= kSplit8MaxCell) return fine ? 8u : ((n_c + 7u) / 8u) * 8u;        // fine: tiny problems need more items
+  if (n_c <= kSplitMaxCell) return fine ? 8u : 48u;
   return n_c <= 64u ? 64u : 128u;
 }
 
@@ -100,7 +103,8 @@ __global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__
       const unsigned long long nchunk = (S + kSrcChunk - 1) / kSrcChunk;
       it = ntile * nchunk;
       w = (unsigned long long)n_c * S;
-      slots = ntile * tpi * ((S + 3ull) & ~3ull);
+      const unsigned long long sp = (n_c <= kSplit8MaxCell || (fine && n_c <= kSplitMaxCell)) ? 7ull : (n_c <= kSplitMaxCell ? 3ull : 0ull);
+      slots = ntile * tpi * ((S + sp) & ~sp);
       nmax = n_c;
     }
     items[c] = it;
@@ -252,8 +256,11 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
     }
     __syncwarp();
     // ---- pair loop: every source of the tile against the lane's 2*TP targets
-    const int cnt = (int)min((uint32_t)kSrcTile, (p1 - tile + 3u) & ~3u);
-#pragma unroll 4
+    const int cnt = (int)min((uint32_t)kSrcTile, (p1 - tile + (uint32_t)(S - 1)) & ~(uint32_t)(S - 1));
+    // unrolled to about 8 packed-pair bodies per trip: the variants run side by side on one SM sub-partition (cells of
+    // 20..46 particles pick four of them), and bodies of 20 packed pairs each (7 KB of code per variant) thrashed the
+    // instruction cache -- FMA-pipe utilisation fell from 83 % to 63 %
+#pragma unroll (TP >= 3 ? 2 : 4)
     for (int j = (S > 1 ? lane / (32 / S) : 0); j < cnt; j += S) {
       // one LDS.128 per source; the packed instructions broadcast the scalar to both halves (R.F32 operand form)
       const float4 sv = ws.src[j];
@@ -384,12 +391,18 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
 
     const uint32_t p0 = (uint32_t)min(chunk * (unsigned long long)kSrcChunk, (unsigned long long)S), p1 = min(S, p0 + kSrcChunk);
     const uint32_t tb = cs0 + tile * tpi, te = min(cs1, tb + tpi);
-    if (n_c <= 16u || (fc.fine_items && n_c <= kSplitMaxCell))
-      process_item<1, kUniformMass, kSplit>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+    if (n_c <= 8u || (fc.fine_items && n_c <= kSplitMaxCell))
+      process_item<1, kUniformMass, 8>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+    else if (n_c <= 16u)
+      process_item<2, kUniformMass, 8>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+    else if (n_c <= 24u)
+      process_item<3, kUniformMass, 8>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
     else if (n_c <= 32u)
-      process_item<2, kUniformMass, kSplit>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+      process_item<4, kUniformMass, 8>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+    else if (n_c <= kSplit8MaxCell)
+      process_item<5, kUniformMass, 8>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
     else if (n_c <= kSplitMaxCell)
-      process_item<3, kUniformMass, kSplit>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+      process_item<3, kUniformMass, 4>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
     else if (n_c <= 64u)
       process_item<1, kUniformMass, 1>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
     else
