@@ -231,7 +231,8 @@ int32_t srpp_subcycle(srpp_ctx* ctx, float* pos_mass, float* vel, float* acc, fl
 /* End-to-end convenience for callers holding HOST arrays: copies pos_mass_host[4n] (and vel_host[4n] if
  * not NULL) to the device, builds the mesh, computes accelerations, optionally kicks (vel_host != NULL:
  * v <- v + kdt*a, copied back), copies acc back to acc_host[4n].  Device scratch for the particle arrays
- * is taken from `device_scratch` (>= 48*n bytes, caller-owned device memory).  Synchronises. */
+ * is taken from `device_scratch` (>= 48*n bytes, caller-owned device memory).  The velocity upload and the download
+ * of the accelerations run on a second stream and overlap the kernels (host buffers should be pinned).  Synchronises. */
 int32_t srpp_step_host(srpp_ctx* ctx, const float* pos_mass_host, float* vel_host, float* acc_host,
                        float kdt, int64_t n, void* device_scratch, size_t device_scratch_bytes);
 

@@ -226,6 +226,9 @@ void srpp_destroy(srpp_ctx* c) {
     if (c->ev[i]) cudaEventDestroy(c->ev[i]);
   for (int i = 0; i < 2; ++i)
     if (c->ev_sub[i]) cudaEventDestroy(c->ev_sub[i]);
+  for (int i = 0; i < 3; ++i)
+    if (c->ev_copy[i]) cudaEventDestroy(c->ev_copy[i]);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   free_block_plan(c);
   delete c;
 }
@@ -394,26 +397,45 @@ int32_t srpp_stream(srpp_ctx* c, float* pos_mass, const float* vel, float dt, in
 int32_t srpp_step_host(srpp_ctx* c, const float* pos_mass_host, float* vel_host, float* acc_host, float kdt,
                        int64_t n, void* device_scratch, size_t device_scratch_bytes) {
   if (!c || n < 0 || n >= ((int64_t)1 << 31) || (n > 0 && (!pos_mass_host || !acc_host || !device_scratch))) return SRPP_ERR_INVALID_ARG;
+  if (const int32_t d = check_device(c)) return d;
   const size_t bytes = 16 * (size_t)n;
   if (device_scratch_bytes < 3 * bytes || ((uintptr_t)device_scratch & 15u)) return SRPP_ERR_WORKSPACE;
   float* d_pos = (float*)device_scratch;
   float* d_acc = (float*)((char*)device_scratch + bytes);
   float* d_vel = (float*)((char*)device_scratch + 2 * bytes);
-  cudaError_t e = cudaMemcpyAsync(d_pos, pos_mass_host, bytes, cudaMemcpyHostToDevice, c->stream);
-  if (e == cudaSuccess && vel_host) e = cudaMemcpyAsync(d_vel, vel_host, bytes, cudaMemcpyHostToDevice, c->stream);
+  // Copies overlap the kernels: the velocities travel on a second stream while the mesh is built and the forces are
+  // evaluated (they are needed only by the kick), and the accelerations travel back while the kick runs.
+  cudaError_t e = cudaSuccess;
+  if (!c->copy_stream) {
+    e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    for (int i = 0; i < 3 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&c->ev_copy[i], cudaEventDisableTiming);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+  }
+  e = cudaEventRecord(c->ev_copy[0], c->stream);                  // the previous use of the scratch is over
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(c->copy_stream, c->ev_copy[0], 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_pos, pos_mass_host, bytes, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess && vel_host) {
+    e = cudaMemcpyAsync(d_vel, vel_host, bytes, cudaMemcpyHostToDevice, c->copy_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(c->ev_copy[1], c->copy_stream);
+  }
   if (e != cudaSuccess) return cuda_fail(c, e);
   int32_t rc = srpp_build_mesh(c, d_pos, n);
-  if (rc != SRPP_OK) return rc;
-  rc = srpp_accel(c, d_acc);
-  if (rc != SRPP_OK) return rc;
+  if (rc == SRPP_OK) rc = srpp_accel(c, d_acc);
+  if (rc != SRPP_OK) { cudaStreamSynchronize(c->copy_stream); return rc; }
+  e = cudaEventRecord(c->ev_copy[2], c->stream);                  // accelerations complete
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(c->copy_stream, c->ev_copy[2], 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(acc_host, d_acc, bytes, cudaMemcpyDeviceToHost, c->copy_stream);
+  if (e != cudaSuccess) return cuda_fail(c, e);
   if (vel_host) {
+    e = cudaStreamWaitEvent(c->stream, c->ev_copy[1], 0);         // velocities have arrived
+    if (e != cudaSuccess) return cuda_fail(c, e);
     rc = srpp_kick(c, d_vel, d_acc, kdt, n);
-    if (rc != SRPP_OK) return rc;
+    if (rc != SRPP_OK) { cudaStreamSynchronize(c->copy_stream); return rc; }
     e = cudaMemcpyAsync(vel_host, d_vel, bytes, cudaMemcpyDeviceToHost, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e);
   }
-  e = cudaMemcpyAsync(acc_host, d_acc, bytes, cudaMemcpyDeviceToHost, c->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  e = cudaStreamSynchronize(c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->copy_stream);
   return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
 }
 

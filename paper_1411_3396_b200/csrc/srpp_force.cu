@@ -75,8 +75,8 @@ __device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint
 constexpr uint32_t kSplit8MaxCell = 40;         // <= 5 packed pairs of 8 targets
 constexpr uint32_t kSplitMaxCell = 48;          // <= 3 packed pairs of 16 targets
 __device__ __forceinline__ uint32_t targets_per_item(uint32_t n_c, int fine) {
-  if (n_c <= kSplit8MaxCell) return fine ? 8u : ((n_c + 7u) / 8u) * 8u;        // fine: tiny problems need more items
-  if (n_c <= kSplitMaxCell) return fine ? 8u : 48u;
+  if (n_c <= kSplit8MaxCell) return fine ? min(16u, ((n_c + 7u) / 8u) * 8u) : ((n_c + 7u) / 8u) * 8u;   // fine: tiny problems need more items
+  if (n_c <= kSplitMaxCell) return fine ? 16u : 48u;
   return n_c <= 64u ? 64u : 128u;
 }
 
@@ -391,9 +391,9 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
 
     const uint32_t p0 = (uint32_t)min(chunk * (unsigned long long)kSrcChunk, (unsigned long long)S), p1 = min(S, p0 + kSrcChunk);
     const uint32_t tb = cs0 + tile * tpi, te = min(cs1, tb + tpi);
-    if (n_c <= 8u || (fc.fine_items && n_c <= kSplitMaxCell))
+    if (n_c <= 8u)
       process_item<1, kUniformMass, 8>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
-    else if (n_c <= 16u)
+    else if (n_c <= 16u || (fc.fine_items && n_c <= kSplitMaxCell))
       process_item<2, kUniformMass, 8>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
     else if (n_c <= 24u)
       process_item<3, kUniformMass, 8>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);

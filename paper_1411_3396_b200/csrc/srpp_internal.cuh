@@ -135,6 +135,8 @@ struct srpp_ctx {
   int64_t status_n_movers;
   int64_t m_cap;             // movers the second set is sized for (n/4): beyond it the re-bin falls back to a full build
   uint64_t rebin_incremental, rebin_full, last_movers;   // counters (srpp_get_stats)
+  cudaStream_t copy_stream;  // srpp_step_host: second stream for the copies that overlap the kernels
+  cudaEvent_t ev_copy[3];
   cudaEvent_t ev_sub[2];     // timing of the re-bins inside srpp_subcycle
   float rebin_ms_sum, subkick_ms_sum; int rebin_count;
   uint32_t* sort_ctl;        // tile tickets + global digit histograms (cleared by every build)
