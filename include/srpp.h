@@ -121,6 +121,14 @@ int32_t srpp_get_mesh(const srpp_ctx* ctx, const uint32_t** cell_start, const ui
  * per-item fp32 partial sums folded into fp64 accumulators.  Asynchronous on the stream. */
 int32_t srpp_accel(srpp_ctx* ctx, float* acc);
 
+/* A5-A7 in one call: srpp_accel followed by srpp_kick(vel, acc, kdt) on the same n particles, with the kick fused into
+ * the write-back (one pass over acc and vel instead of a scattered write of acc and a second pass that re-reads it).
+ * Results are bit-identical to the two separate calls.  acc, vel: device float4[n], n = particles of the last mesh.
+ * For n >= 2^22 the write-back is bucketed (two coalesced passes through a 16 n-byte buffer of the workspace) because
+ * the destinations perm[k] have no locality.  Asynchronous on the stream.
+ * Errors: INVALID_ARG (null / misaligned pointer, non-finite kdt), STATE, CUDA. */
+int32_t srpp_accel_kick(srpp_ctx* ctx, float* acc, float* vel, float kdt);
+
 /* Counters of the last srpp_accel (synchronises the stream). */
 int32_t srpp_get_stats(srpp_ctx* ctx, srpp_stats* stats_host);
 

@@ -18,7 +18,7 @@ SRPP_OK = 0
 STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "GEOMETRY", -3: "DOMAIN", -4: "WORKSPACE", -5: "STATE", -6: "CUDA"}
 
 EXPORTS = ("srpp_version", "srpp_default_poly", "srpp_workspace_bytes", "srpp_create", "srpp_destroy",
-           "srpp_build_mesh", "srpp_get_mesh", "srpp_accel", "srpp_get_stats", "srpp_kick", "srpp_stream",
+           "srpp_build_mesh", "srpp_get_mesh", "srpp_accel", "srpp_accel_kick", "srpp_get_stats", "srpp_kick", "srpp_stream",
            "srpp_step_host", "srpp_strerror", "srpp_last_cuda_error", "srpp_set_timing", "srpp_get_timings",
            "srpp_probe_fp32", "srpp_set_boundary", "srpp_mbp_workspace_bytes", "srpp_mbp", "srpp_subcycle",
            "srpp_blocks_workspace_bytes", "srpp_blocks_init", "srpp_accel_blocks", "srpp_get_blocks")
@@ -83,6 +83,8 @@ def load() -> C.CDLL:
     L.srpp_get_mesh.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     L.srpp_accel.restype = i32
     L.srpp_accel.argtypes = [vp, vp]
+    L.srpp_accel_kick.restype = i32
+    L.srpp_accel_kick.argtypes = [vp, vp, vp, f32]
     L.srpp_get_stats.restype = i32
     L.srpp_get_stats.argtypes = [vp, C.POINTER(SrppStats)]
     L.srpp_kick.restype = i32
@@ -243,6 +245,19 @@ class Solver:
         if acc.shape[0] != self.n:
             raise ValueError("acc has %d rows, mesh has %d particles" % (acc.shape[0], self.n))
         self._check(self.lib.srpp_accel(self._ctx, acc.data_ptr()), "srpp_accel")
+        return acc
+
+    def accel_kick(self, vel, kdt: float, acc=None):
+        """srpp_accel_kick: accelerations (caller's order) and v <- fmaf(a, kdt, v) in one call; returns acc."""
+        torch = self._torch
+        if self.n < 0:
+            self._check(-5, "srpp_accel_kick")
+        if acc is None:
+            acc = torch.empty((self.n, 4), dtype=torch.float32, device=self.device)
+        self._f4(acc, "acc"), self._f4(vel, "vel")
+        if acc.shape[0] != self.n or vel.shape[0] != self.n:
+            raise ValueError("acc / vel rows differ from the mesh's %d particles" % self.n)
+        self._check(self.lib.srpp_accel_kick(self._ctx, acc.data_ptr(), vel.data_ptr(), float(kdt)), "srpp_accel_kick")
         return acc
 
     def get_stats(self) -> dict:

@@ -21,6 +21,7 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   const size_t o_flags = take(sizeof(DevFlags));
   const size_t o_v0 = take(4 * nn), o_v1 = take(4 * nn), o_v2 = take(4 * nn), o_keys = take(4 * nn);
   const size_t o_ctl = take(sort_ctl_bytes());
+  const size_t o_ucur = take(4 * 256);
   const size_t o_status = take(8 * (size_t)kSortMaxBins * (nn / kPassTile + 1));   // [tiles][bins] look-back words
   const size_t o_cs = take(4 * (ncells + 1));
   const size_t o_sorted = take(16 * nn);
@@ -58,6 +59,7 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
     c->m_keys = (uint32_t*)(b + o_mkeys); c->m_cell_start = (uint32_t*)(b + o_mcs);
     c->m_cap = (int64_t)mcap;
     c->sort_ctl = (uint32_t*)(b + o_ctl);
+    c->unsort_cursor = (uint32_t*)(b + o_ucur);
     if (c->sort_status != (unsigned long long*)(b + o_status)) c->status_n = 0;   // the array moved: clear before use
     c->sort_status = (unsigned long long*)(b + o_status);
     c->cell_start = (uint32_t*)(b + o_cs);
@@ -362,6 +364,15 @@ int32_t srpp_accel(srpp_ctx* c, float* acc) {
   return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
 }
 
+int32_t srpp_accel_kick(srpp_ctx* c, float* acc, float* vel, float kdt) {
+  if (!c) return SRPP_ERR_INVALID_ARG;
+  if (c->n < 0) return SRPP_ERR_STATE;
+  if ((c->n > 0 && (!acc || !vel)) || misaligned16(acc) || misaligned16(vel) || !isfinite(kdt)) return SRPP_ERR_INVALID_ARG;
+  if (const int32_t d = check_device(c)) return d;
+  const cudaError_t e = launch_accel(c, (float4*)acc, (float4*)vel, kdt);
+  return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);
+}
+
 int32_t srpp_get_stats(srpp_ctx* c, srpp_stats* s) {
   if (!c || !s) return SRPP_ERR_INVALID_ARG;
   if (c->n < 0) return SRPP_ERR_STATE;
@@ -420,20 +431,22 @@ int32_t srpp_step_host(srpp_ctx* c, const float* pos_mass_host, float* vel_host,
   }
   if (e != cudaSuccess) return cuda_fail(c, e);
   int32_t rc = srpp_build_mesh(c, d_pos, n);
-  if (rc == SRPP_OK) rc = srpp_accel(c, d_acc);
   if (rc != SRPP_OK) { cudaStreamSynchronize(c->copy_stream); return rc; }
-  e = cudaEventRecord(c->ev_copy[2], c->stream);                  // accelerations complete
+  if (n > 0) {
+    // force kernel, then the write-back with the kick fused into it (A6 + A7 in one pass over acc and vel)
+    if (c->timing) cudaEventRecord(c->ev[kEvAccel0], c->stream);
+    e = launch_accel_sorted(c);
+    if (e == cudaSuccess && vel_host) e = cudaStreamWaitEvent(c->stream, c->ev_copy[1], 0);     // velocities have arrived
+    if (e == cudaSuccess) e = launch_write_back(c, (float4*)d_acc, vel_host ? (float4*)d_vel : nullptr, kdt);
+    if (c->timing) { cudaEventRecord(c->ev[kEvAccel1], c->stream); c->ev_accel_valid = true; }
+    if (e != cudaSuccess) { cudaStreamSynchronize(c->copy_stream); return cuda_fail(c, e); }
+  }
+  // the two downloads run side by side: accelerations on the copy stream, velocities on the solver's stream
+  e = cudaEventRecord(c->ev_copy[2], c->stream);
   if (e == cudaSuccess) e = cudaStreamWaitEvent(c->copy_stream, c->ev_copy[2], 0);
   if (e == cudaSuccess) e = cudaMemcpyAsync(acc_host, d_acc, bytes, cudaMemcpyDeviceToHost, c->copy_stream);
+  if (e == cudaSuccess && vel_host) e = cudaMemcpyAsync(vel_host, d_vel, bytes, cudaMemcpyDeviceToHost, c->stream);
   if (e != cudaSuccess) return cuda_fail(c, e);
-  if (vel_host) {
-    e = cudaStreamWaitEvent(c->stream, c->ev_copy[1], 0);         // velocities have arrived
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    rc = srpp_kick(c, d_vel, d_acc, kdt, n);
-    if (rc != SRPP_OK) { cudaStreamSynchronize(c->copy_stream); return rc; }
-    e = cudaMemcpyAsync(vel_host, d_vel, bytes, cudaMemcpyDeviceToHost, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-  }
   e = cudaStreamSynchronize(c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->copy_stream);
   return e == cudaSuccess ? SRPP_OK : cuda_fail(c, e);

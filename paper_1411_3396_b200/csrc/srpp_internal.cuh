@@ -29,6 +29,7 @@ constexpr int kForceWarps = kForceThreads / 32;
 constexpr int kSrcTile = 128;                 // sources staged per warp-private smem tile (float4 each)
 constexpr int kSrcChunk = 1024;               // sources per work item (fp32 partial-sum length)
 constexpr int kMaxSeg = 18;                   // 9 (dy,dz) rows x up to 2 x-segments (periodic wrap)
+constexpr int64_t kUnsortMinN = (int64_t)1 << 22;   // write-back: below this acc and vel sit in L2 and the direct scatter wins
 
 // timing events: mesh begin/end, accel begin, force-kernel begin/end, accel end
 enum { kEvMesh0 = 0, kEvMesh1, kEvAccel0, kEvForce0, kEvForce1, kEvAccel1, kNumEvents };
@@ -107,6 +108,8 @@ struct srpp_ctx {
   int sort_blocks;
   int sort_blocks_per_sm;
   bool sort_attr_set;
+  bool unsort_attr_set;
+  uint32_t* unsort_cursor;   // [256] run cursors of the bucketed write-back (srpp_force.cu)
   bool uniform_mass;
   float mass0;
   // workspace carve-up (device pointers)
@@ -178,9 +181,10 @@ cudaError_t launch_build_mesh(srpp_ctx* c, const float4* pos_mass, int64_t n);
 cudaError_t sort_by_cell(srpp_ctx* c, SortBufs& sb, const float4* pos_mass, int64_t n);
 void plan_sort(int32_t ncells, int* passes, int* digit_bits);
 // srpp_force.cu
-cudaError_t launch_accel(srpp_ctx* c, float4* acc);            // force + write-back
+// force + write-back (+ the kick of A7 fused into the write-back when vel != nullptr)
+cudaError_t launch_accel(srpp_ctx* c, float4* acc, float4* vel = nullptr, float kdt = 0.f);
 cudaError_t launch_accel_sorted(srpp_ctx* c);                  // force only: fp64 accumulators in sorted order
-cudaError_t launch_write_back(srpp_ctx* c, float4* acc);       // A6
+cudaError_t launch_write_back(srpp_ctx* c, float4* acc, float4* vel = nullptr, float kdt = 0.f);   // A6 (+ A7)
 // srpp_subcycle.cu
 cudaError_t launch_subcycle(srpp_ctx* c, float4* pos_mass, float4* vel, float4* acc, float dt, float kdt, int nsub,
                             int64_t n, int32_t* status_out);

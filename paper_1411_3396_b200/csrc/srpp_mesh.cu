@@ -153,11 +153,20 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_prepass(const float4* __r
 // kind 1: the tile's own count of the digit (aggregate); kind 2: inclusive prefix over tiles 0..t.  The epoch
 // changes with every pass of every build, so the array never needs clearing between passes.
 constexpr uint32_t kStatAgg = 1u, kStatPrefix = 2u;
-constexpr int kPassThreads = 1024;                      // 32 warps, one CTA per SM: the pass is bound by shared-memory
+#ifndef SRPP_PASS_THREADS
+#define SRPP_PASS_THREADS 1024
+#endif
+#ifndef SRPP_PASS_CTAS
+#define SRPP_PASS_CTAS 1
+#endif
+#ifndef SRPP_LOOK_WINDOW
+#define SRPP_LOOK_WINDOW 4
+#endif
+constexpr int kPassThreads = SRPP_PASS_THREADS;         // 32 warps, one CTA per SM: the pass is bound by shared-memory
 constexpr int kPassWarps = kPassThreads / 32;           // wavefronts and the latency between its phases, not by DRAM
 constexpr int kPassItems = kPassTile / kPassThreads;    // (2 CTAs x 512 threads x 2048-element tiles measured slower)
-constexpr int kPassCtasPerSm = 1;
-constexpr int kLookWindow = 4;                          // status words of earlier tiles read per round trip
+constexpr int kPassCtasPerSm = SRPP_PASS_CTAS;
+constexpr int kLookWindow = SRPP_LOOK_WINDOW;                          // status words of earlier tiles read per round trip
 
 // Dynamic shared memory of a pass (bytes), for nbins bins.
 __host__ __device__ inline size_t sort_pass_smem(int nbins, bool packed) {

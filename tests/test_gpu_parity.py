@@ -328,6 +328,41 @@ def test_kick_stream_bit_exact(oracle_mod, gpu):
     sol.build_mesh(dx)          # stream keeps the domain precondition
 
 
+@pytest.mark.parametrize("n,ncell", [(50021, (6, 5, 7)),                  # direct write-back (acc and vel sit in L2)
+                                     ((1 << 22) + 4099, (50, 50, 51))])   # bucketed write-back: ragged last tile and bucket
+def test_accel_kick_fused_write_back(oracle_mod, gpu, n, ncell):
+    """srpp_accel_kick (A5-A7 in one call, kick fused into the write-back): accelerations of ALL
+    particles against the oracle, velocities bit-exact against orc_kick fed those accelerations, and bit-identical to
+    srpp_accel + srpp_kick.  acc is pre-filled with NaN: every destination must be written exactly once."""
+    torch, binding = gpu
+    rng = np.random.default_rng(n)
+    box = tuple(3.2 * c for c in ncell)
+    pos = np.ones((n, 4), dtype=np.float32)
+    pos[:, :3] = (rng.random((n, 3)) * np.asarray(box)).astype(np.float32)
+    pos[:, :3] = np.minimum(pos[:, :3], np.nextafter(np.asarray(box, dtype=np.float32), 0))
+    v0 = rng.normal(size=(n, 4)).astype(np.float32)
+    sol = _solver(gpu, box, ncell, 0.1, n)
+    d = torch.from_numpy(pos).cuda()
+    sol.build_mesh(d)
+    d_vel = torch.from_numpy(v0.copy()).cuda()
+    d_acc = torch.full((n, 4), float("nan"), dtype=torch.float32, device="cuda")
+    sol.accel_kick(d_vel, 0.0125, acc=d_acc)
+    torch.cuda.synchronize()
+    a = d_acc.cpu().numpy()
+    assert np.all(np.isfinite(a)) and np.all(a[:, 3] == 0.0)
+    per, glob = _check_accel(oracle_mod, a, pos, box, 0.1, label="accel_kick n=%d" % n)
+    assert np.array_equal(d_vel.cpu().numpy().view(np.uint32), oracle_mod.kick(v0, a, 0.0125).view(np.uint32))
+    # the two separate calls give the same bits (same force kernel; fp64 folds of <= 1 item per target at this density)
+    d_acc2 = torch.full((n, 4), float("nan"), dtype=torch.float32, device="cuda")
+    sol.accel(d_acc2)
+    d_vel2 = torch.from_numpy(v0.copy()).cuda()
+    sol.kick(d_vel2, d_acc2, 0.0125)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_acc2.cpu().numpy().view(np.uint32), a.view(np.uint32))
+    assert np.array_equal(d_vel2.cpu().numpy().view(np.uint32), d_vel.cpu().numpy().view(np.uint32))
+    print("accel_kick n=%d: per-particle max %.3e, global L2 %.3e" % (n, per, glob))
+
+
 def test_subcycle_fixed_positions(oracle_mod, gpu):
     """Config-4 reading (R16): 5 x {build mesh, accel, kick} on fixed positions; identical accelerations each step
     are not required bit-wise (atomic order) but v5 = 5 kicks of the oracle's a within tolerance."""
