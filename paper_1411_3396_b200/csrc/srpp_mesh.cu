@@ -95,6 +95,19 @@ __device__ __forceinline__ void st_keep_u32(uint32_t* p, uint32_t v, uint64_t po
 __device__ __forceinline__ void st_keep_f4(float4* p, float4 v, uint64_t pol) {
   asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
 }
+// TMA bulk store of one per-digit run, shared -> global (16-byte aligned, a multiple of 16 bytes), with an L2 policy
+__device__ __forceinline__ void bulk_store(void* gmem_dst, const void* smem_src, uint32_t bytes, uint64_t pol) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(gmem_dst),
+               "r"((uint32_t)__cvta_generic_to_shared(smem_src)), "r"(bytes), "l"(pol) : "memory");
+}
+// TMA prefetch of a contiguous global range into L2 (no registers, no shared memory); bytes a multiple of 16
+__device__ __forceinline__ void bulk_prefetch_l2(const void* gmem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
   unsigned long long v; asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory"); return v;
 }
@@ -154,10 +167,16 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_prepass(const float4* __r
 // changes with every pass of every build, so the array never needs clearing between passes.
 constexpr uint32_t kStatAgg = 1u, kStatPrefix = 2u;
 #ifndef SRPP_PASS_THREADS
-#define SRPP_PASS_THREADS 1024
+#define SRPP_PASS_THREADS 512
 #endif
 #ifndef SRPP_PASS_CTAS
-#define SRPP_PASS_CTAS 1
+#define SRPP_PASS_CTAS 2
+#endif
+#ifndef SRPP_L2_PREFETCH
+#define SRPP_L2_PREFETCH 1
+#endif
+#ifndef SRPP_BULK_STORE
+#define SRPP_BULK_STORE 1
 #endif
 #ifndef SRPP_LOOK_WINDOW
 #define SRPP_LOOK_WINDOW 4
@@ -193,7 +212,11 @@ __host__ __device__ inline size_t sort_pass_smem(int nbins, bool packed) {
 //   * the elements go to their slot of the digit-ordered tile in shared memory and are written out as per-digit runs,
 //     consecutive threads -> consecutive addresses (stores of single 16-byte elements straight to their final place
 //     were measured at a third of this speed).  Four CTA barriers per tile.
-template <bool kPacked>
+// kBulk (equal masses, every pass but the last): the per-digit runs of the digit-ordered tile leave shared memory as
+// TMA bulk stores, one per digit thread (cp.async.bulk: 128 runs of ~512 bytes per tile reach the HBM write rate,
+// measured), so the write-out phase and its barrier disappear: a tile is rank -> scan -> slot store + look-back ->
+// issue, three barriers, and the stores drain while the next tile is ranked.
+template <bool kPacked, bool kBulk>
 __global__ void __launch_bounds__(kPassThreads, kPassCtasPerSm) k_sort_pass(
     const float4* __restrict__ pos_in, const uint32_t* __restrict__ idx_in, float4* __restrict__ pos_out,
     uint32_t* __restrict__ idx_out, uint32_t* __restrict__ keys_out, const float4* __restrict__ pos_orig, int64_t n,
@@ -202,6 +225,7 @@ __global__ void __launch_bounds__(kPassThreads, kPassCtasPerSm) k_sort_pass(
     const DevFlags* __restrict__ flags) {
   // the mode is a device-side fact (found by the prepass): both instantiations are launched, one returns at once
   if ((flags->mass_nonuniform == 0u) != kPacked) return;
+  static_assert(!kBulk || kPacked, "bulk stores carry whole 16-byte elements");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* spos = (float4*)smem_raw;                                        // [kPassTile] digit order
   uint32_t* sidx = (uint32_t*)(spos + kPassTile);                          // [kPassTile]   (!kPacked only)
@@ -228,7 +252,21 @@ __global__ void __launch_bounds__(kPassThreads, kPassCtasPerSm) k_sort_pass(
   // leave them clear)
   if ((int)threadIdx.x < nbins) base[threadIdx.x] = ghist[threadIdx.x];
   for (int q = threadIdx.x; q < kPassWarps * nbins; q += kPassThreads) masks[q] = 0u;
-  if (threadIdx.x == 0) scratch[32] = atomicAdd(ticket, 1u);
+  // Tiles are taken in ticket order, one ahead (a ticket held longer would stall the look-back of every later tile).
+  // The tile a CTA will take after the next one is, in the steady state, about gridDim.x tickets further on: that
+  // tile is pulled into L2 by one TMA prefetch, so that the register loads of whichever CTA gets it find it there.
+  auto prefetch_tile = [&](int64_t tile) {
+    if (SRPP_L2_PREFETCH && tile < ntiles) {
+      const int64_t cnt = min((int64_t)kPassTile, n - tile * kPassTile);
+      bulk_prefetch_l2(pos_in + tile * kPassTile, (uint32_t)cnt * (uint32_t)sizeof(float4));
+      if (!kPacked && !first) bulk_prefetch_l2(idx_in + tile * kPassTile, (uint32_t)((cnt * 4 + 15) & ~15ll));
+    }
+  };
+  if (threadIdx.x == 0) {
+    const uint32_t t0 = atomicAdd(ticket, 1u);
+    scratch[32] = t0;
+    prefetch_tile((int64_t)t0 + gridDim.x);
+  }
   __syncthreads();
   cta_scan_bins<kPassThreads>(base, nbins, scratch);
   int64_t t = scratch[32];
@@ -252,7 +290,11 @@ __global__ void __launch_bounds__(kPassThreads, kPassCtasPerSm) k_sort_pass(
   while (t < ntiles) {
     const int64_t tile = t * kPassTile;
     const int tile_n = (int)min((int64_t)kPassTile, n - tile);
-    if (threadIdx.x == 0) scratch[33] = atomicAdd(ticket, 1u);
+    if (threadIdx.x == 0) {
+      const uint32_t tn = atomicAdd(ticket, 1u);
+      scratch[33] = tn;
+      prefetch_tile((int64_t)tn + gridDim.x);
+    }
     for (int q = lane; q < nbins; q += 32) mycount[q] = 0u;
     __syncwarp();
     // ---- stable ranks inside the warp's 128 consecutive elements
@@ -303,6 +345,7 @@ __global__ void __launch_bounds__(kPassThreads, kPassCtasPerSm) k_sort_pass(
       const uint32_t ts = off + x - cnt_d;
       tstart[d] = ts;
       cnt_keep = cnt_d; ts_keep = ts;
+      if (kBulk) bulk_wait_read();                       // the previous tile's runs have left shared memory
     }
     __syncthreads();                                     // B2: tstart and the prefixes over the warps are ready
     // ---- every element to its slot of the digit-ordered tile
@@ -320,6 +363,10 @@ __global__ void __launch_bounds__(kPassThreads, kPassCtasPerSm) k_sort_pass(
         if (kPacked) v.w = __uint_as_float(idx); else sidx[slot] = idx;
         spos[slot] = v;
       }
+    }
+    if (kBulk) {
+      fence_async_smem();                                // the slot stores become visible to the TMA engine
+      load_tile(t_next);                                 // registers are free again: request the next tile now
     }
     // ---- digit threads: decoupled look-back (the other warps are storing their elements meanwhile)
     if ((int)threadIdx.x < nbins) {
@@ -347,6 +394,14 @@ __global__ void __launch_bounds__(kPassThreads, kPassCtasPerSm) k_sort_pass(
       goff[d] = base[d] + excl - ts_keep;
     }
     __syncthreads();                                     // B3: digit-ordered tile and goff complete
+    if (kBulk) {
+      if ((int)threadIdx.x < nbins) {
+        if (cnt_keep) bulk_store(pos_out + goff[threadIdx.x] + ts_keep, spos + ts_keep, cnt_keep * (uint32_t)sizeof(float4), pol_out);
+        bulk_commit();
+      }
+      t = t_next;
+      continue;                                          // no fourth barrier: see the reuse notes above each structure
+    }
     // ---- next tile's elements are requested now, this tile is written out as per-digit runs meanwhile
     load_tile(t_next);
 #pragma unroll
@@ -370,6 +425,7 @@ __global__ void __launch_bounds__(kPassThreads, kPassCtasPerSm) k_sort_pass(
     t = t_next;
     __syncthreads();                                     // B4: the digit-ordered tile, goff and the ticket word are reused
   }
+  if (kBulk && (int)threadIdx.x < nbins) bulk_wait_all();
 }
 
 // --------------------------------------------------------------- cell_start from run boundaries --
@@ -427,8 +483,9 @@ cudaError_t sort_by_cell(srpp_ctx* c, SortBufs& sb, const float4* pos_mass, int6
 
   const size_t smem_packed = sort_pass_smem(nbins, true), smem_plain = sort_pass_smem(nbins, false);
   if (!c->sort_attr_set) {
-    if ((e = cudaFuncSetAttribute(k_sort_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_pass_smem(kSortMaxBins, true))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_sort_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_pass_smem(kSortMaxBins, false))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_sort_pass<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_pass_smem(kSortMaxBins, true))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_sort_pass<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_pass_smem(kSortMaxBins, true))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_sort_pass<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_pass_smem(kSortMaxBins, false))) != cudaSuccess) return e;
     c->sort_attr_set = true;
   }
   const int64_t tiles = (n + kSortTile - 1) / kSortTile, ptiles = (n + kPassTile - 1) / kPassTile;
@@ -455,8 +512,11 @@ cudaError_t sort_by_cell(srpp_ctx* c, SortBufs& sb, const float4* pos_mass, int6
     const int o = p & 1;
     const int first = p == 0, last = p == passes - 1;
     const uint32_t epoch = ++c->sort_epoch;
-    k_sort_pass<true><<<blocks, kPassThreads, smem_packed, st>>>(pin, iin, posbuf[o], sb.vals[o], sb.keys_out, pos_mass, n, c->geo, shift, nbins, first, last, ghist + (size_t)p * kSortMaxBins, sb.status, tickets + p, epoch, sb.flags);
-    k_sort_pass<false><<<blocks, kPassThreads, smem_plain, st>>>(pin, iin, posbuf[o], sb.vals[o], sb.keys_out, pos_mass, n, c->geo, shift, nbins, first, last, ghist + (size_t)p * kSortMaxBins, sb.status, tickets + p, epoch, sb.flags);
+    if (SRPP_BULK_STORE && !last)
+      k_sort_pass<true, true><<<blocks, kPassThreads, smem_packed, st>>>(pin, iin, posbuf[o], sb.vals[o], sb.keys_out, pos_mass, n, c->geo, shift, nbins, first, last, ghist + (size_t)p * kSortMaxBins, sb.status, tickets + p, epoch, sb.flags);
+    else
+      k_sort_pass<true, false><<<blocks, kPassThreads, smem_packed, st>>>(pin, iin, posbuf[o], sb.vals[o], sb.keys_out, pos_mass, n, c->geo, shift, nbins, first, last, ghist + (size_t)p * kSortMaxBins, sb.status, tickets + p, epoch, sb.flags);
+    k_sort_pass<false, false><<<blocks, kPassThreads, smem_plain, st>>>(pin, iin, posbuf[o], sb.vals[o], sb.keys_out, pos_mass, n, c->geo, shift, nbins, first, last, ghist + (size_t)p * kSortMaxBins, sb.status, tickets + p, epoch, sb.flags);
     pin = posbuf[o]; iin = sb.vals[o];
   }
   const int grid_ew = (int)((n + 2047) / 2048);     // one trip per thread: the loads of all CTAs overlap
