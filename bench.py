@@ -2,7 +2,7 @@
 """bench.py -- throughput of the short-range PP hot path on B200 (contract: see the round prompt / DESIGN.md).
 
 A "step" is one pass of the whole hot path over one batch of synthetic input:
-    srpp_build_mesh (A1-A4)  ->  srpp_accel (A5-A6)  ->  srpp_kick (A7)
+    srpp_build_mesh (A1-A4)  ->  srpp_accel_kick (A5 force, A6 write-back with the A7 kick fused into it)
 on the workload BASELINE.json's target is quoted on: configs[3], the clustered 2^25-particle per-node load
 (`--config 4`; configs are numbered 1..5 as in SURVEY.md).  Metric: candidate pair interactions per second,
 W / t_step with W = sum_c n_c * sum_{c' in 27-stencil(c)} n_c' (depends on the input only).
@@ -272,8 +272,7 @@ def run_product(args, w):
 
     def step():
         sol.build_mesh(d_pos)
-        sol.accel(d_acc)
-        sol.kick(d_vel, d_acc, kdt)
+        sol.accel_kick(d_vel, kdt, acc=d_acc)       # A5 + A6 + A7: accelerations in the caller's order and v += kdt * a
 
     for _ in range(args.warmup):
         step()
@@ -340,7 +339,7 @@ def run_product(args, w):
         "config": {"workload": w.name, "baseline_config": "BASELINE.json configs[%d]" % (args.config - 1),
                    "n_particles": n, "box": list(w.box), "ncell": list(w.ncell), "rcut": w.rcut, "eps": w.eps,
                    "candidate_pairs_W": W, "max_cell_count": stats1["max_cell_count"],
-                   "step": "build_mesh + accel + kick", "parallelism": "replicas only (no exchange step)",
+                   "step": "build_mesh + accel_kick (force, write-back and kick; same results as accel + kick)", "parallelism": "replicas only (no exchange step)",
                    "l2": "inputs larger than L2 (16 B x N = %d MiB per array)" % (16 * n >> 20)},
         "clocks": clk, "e2e": e2e, "gpu_launches": launches,
         "roofline": {"bound": "alu", "kernel": "k_pp_force", "achieved": achieved, "peak": peak_tflops,
@@ -355,6 +354,9 @@ def run_product(args, w):
                      "frac_of_probe_ffma2": (achieved / probe["ffma2_tflops"]) if achieved else None},
         "phases": {"mesh_ms": mesh_avg_ms, "accel_ms": float(np.mean(accel_ms)) if accel_ms else None,
                    "force_ms": force_avg_ms,
+                   "plan_write_back_kick_ms": float(np.mean(accel_ms) - np.mean(force_ms)) if accel_ms else None,
+                   "write_back_kick_kind": "accel_ms - force_ms: work plan (4 small kernels) + bucketed write-back with the "
+                                           "kick fused in; algorithmic bytes 28 read + 16 written (A6) + 32 (A7) per particle",
                    "accel_pairs_per_s": W / (np.mean(accel_ms) * 1e-3) if accel_ms else None,
                    "binning_gbs": bin_bytes / (mesh_avg_ms * 1e-3) / 1e9 if mesh_avg_ms else None,
                    "binning_frac_of_hbm": (bin_bytes / (mesh_avg_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]) if mesh_avg_ms else None,

@@ -21,7 +21,7 @@ size_t workspace_layout(const srpp_params& p, int64_t n, srpp_ctx* c) {
   const size_t o_flags = take(sizeof(DevFlags));
   const size_t o_v0 = take(4 * nn), o_v1 = take(4 * nn), o_v2 = take(4 * nn), o_keys = take(4 * nn);
   const size_t o_ctl = take(sort_ctl_bytes());
-  const size_t o_ucur = take(4 * 256);
+  const size_t o_ucur = take(unsort_cursor_bytes(n));
   const size_t o_status = take(8 * (size_t)kSortMaxBins * (nn / kPassTile + 1));   // [tiles][bins] look-back words
   const size_t o_cs = take(4 * (ncells + 1));
   const size_t o_sorted = take(16 * nn);

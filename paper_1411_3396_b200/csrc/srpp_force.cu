@@ -449,24 +449,30 @@ __global__ void __launch_bounds__(256) k_write_back(const double* __restrict__ a
 }
 
 // Bucketed form (n >= kUnsortMinN).  perm is a random permutation of the caller's order in the worst case,
-// so the direct scatter touches one 32-byte DRAM sector per 16-byte store with no locality: measured 1.43 ms for 2^25
-// particles, 0.145 of the HBM copy rate.  Two coalesced passes instead:
-//   k_unsort_partition  tiles of 4096 sorted slots; element = (ax, ay, az, destination index in the .w lane); bucket =
-//                       destination >> shift (<= 256 buckets of 2^shift consecutive destinations: exactly 2^shift
-//                       elements each, perm being a permutation, so the bucket bases are known without a histogram);
-//                       unordered inside a bucket (ranks from shared-memory atomics, one global atomic per tile and
-//                       bucket reserves the run) -- the order is irrelevant, pass 2 stores every element at its own index;
-//   k_unsort_apply      reads the buckets in order; the scattered stores (and, with the kick fused, the loads and stores of
-//                       vel) of the CTAs running at one time fall into a few windows of 2^shift x 16 bytes that stay in
-//                       L2 until their sectors are complete.
+// so the direct scatter touches one 32-byte DRAM sector per 16-byte store with no locality (measured: 1.43 ms for 2^25
+// particles, 0.145 of the HBM copy rate; a scatter into L2-sized windows is no better -- every 16-byte store to a
+// sector that is not resident costs a DRAM fill and the sector is written back twice).  Instead the elements
+// (ax, ay, az, destination index in the .w lane) are radix-partitioned by DESTINATION, most significant digit first,
+// in two (n <= 2^28) or three coalesced passes down to windows of 4096 consecutive destinations:
+//   k_unsort_partition  tiles of 4096 elements; bucket = destination >> shift.  perm is a permutation, so bucket b
+//                       holds exactly the destinations [b << shift, (b + 1) << shift): its place in the output is known
+//                       without a histogram and one global atomic per tile and bucket reserves the tile's run in it.
+//                       Unordered inside a bucket (ranks from shared-memory atomics): the order does not matter.
+//   k_unsort_final      one CTA per window: the 4096 elements are placed at (destination & 4095) in shared memory and
+//                       leave as a linear stream -- with the kick of A7 fused in, vel is read and written linearly too.
 constexpr int kUnsortThreads = 512;
 constexpr int kUnsortTile = 4096;
+constexpr int kUnsortWinBits = 12;                        // final windows: 4096 destinations = one shared-memory tile
 constexpr int kUnsortItems = kUnsortTile / kUnsortThreads;
 constexpr int kUnsortMaxBins = 256;
 
+// kFromAcc: first level (reads the fp64 accumulators and perm); else reads the previous level's elements.
+// prev_shift: the input is already grouped in windows of 2^prev_shift destinations (31: the whole array).
+template <bool kFromAcc>
 __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_partition(
-    const double* __restrict__ acc64, const uint32_t* __restrict__ perm, int64_t n, float scale, int shift, int nbins,
-    uint32_t* __restrict__ cursor /*[nbins], cleared*/, float4* __restrict__ out) {
+    const double* __restrict__ acc64, const uint32_t* __restrict__ perm, const float4* __restrict__ in, int64_t n,
+    float scale, int prev_shift, int shift, uint32_t* __restrict__ cursor /*[n >> shift, +1], cleared*/,
+    float4* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* stile = (float4*)smem_raw;                       // [kUnsortTile] bucket order
   uint32_t* cnt = (uint32_t*)(stile + kUnsortTile);        // [kUnsortMaxBins]
@@ -475,10 +481,12 @@ __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_partition(
   uint32_t* wsum = gbase + kUnsortMaxBins;                 // [32]
   const double s = (double)scale;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const uint32_t lmask = (1u << (prev_shift - shift)) - 1u;      // buckets per input window (<= kUnsortMaxBins)
   const int64_t ntiles = (n + kUnsortTile - 1) / kUnsortTile;
   for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
     const int64_t base = t * kUnsortTile;
     const int tile_n = (int)min((int64_t)kUnsortTile, n - base);
+    const uint32_t bucket0 = (uint32_t)(base >> prev_shift) << (prev_shift - shift);   // first bucket of the tile's window
     if ((int)threadIdx.x < kUnsortMaxBins) cnt[threadIdx.x] = 0u;
     __syncthreads();
     float4 v[kUnsortItems];
@@ -489,19 +497,23 @@ __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_partition(
       v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
       if (e < tile_n) {
         const int64_t k = base + e;
-        const uint32_t dst = __ldcs(&perm[k]);
-        v[u] = make_float4((float)(__ldcs(&acc64[3 * k + 0]) * s), (float)(__ldcs(&acc64[3 * k + 1]) * s),
-                           (float)(__ldcs(&acc64[3 * k + 2]) * s), __uint_as_float(dst));
+        if (kFromAcc) {
+          const uint32_t dst = __ldcs(&perm[k]);
+          v[u] = make_float4((float)(__ldcs(&acc64[3 * k + 0]) * s), (float)(__ldcs(&acc64[3 * k + 1]) * s),
+                             (float)(__ldcs(&acc64[3 * k + 2]) * s), __uint_as_float(dst));
+        } else {
+          v[u] = __ldcs(&in[k]);
+        }
       }
     }
 #pragma unroll
     for (int u = 0; u < kUnsortItems; ++u)
-      if (u * kUnsortThreads + (int)threadIdx.x < tile_n) rk[u] = atomicAdd(&cnt[__float_as_uint(v[u].w) >> shift], 1u);
+      if (u * kUnsortThreads + (int)threadIdx.x < tile_n) rk[u] = atomicAdd(&cnt[(__float_as_uint(v[u].w) >> shift) & lmask], 1u);
     __syncthreads();
     // bucket threads: reserve the tile's run in every bucket, exclusive scan of the counts over the buckets
     if ((int)threadIdx.x < kUnsortMaxBins) {
       const uint32_t c = cnt[threadIdx.x];
-      gbase[threadIdx.x] = c ? atomicAdd(&cursor[threadIdx.x], c) : 0u;
+      gbase[threadIdx.x] = c ? atomicAdd(&cursor[bucket0 + threadIdx.x], c) : 0u;
       uint32_t x = c;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
@@ -514,48 +526,68 @@ __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_partition(
     __syncthreads();
 #pragma unroll
     for (int u = 0; u < kUnsortItems; ++u)
-      if (u * kUnsortThreads + (int)threadIdx.x < tile_n) stile[tstart[__float_as_uint(v[u].w) >> shift] + rk[u]] = v[u];
+      if (u * kUnsortThreads + (int)threadIdx.x < tile_n) stile[tstart[(__float_as_uint(v[u].w) >> shift) & lmask] + rk[u]] = v[u];
     __syncthreads();
 #pragma unroll
     for (int u = 0; u < kUnsortItems; ++u) {
       const int q = u * kUnsortThreads + threadIdx.x;
       if (q < tile_n) {
         const float4 e = stile[q];
-        const uint32_t b = __float_as_uint(e.w) >> shift;
-        out[((size_t)b << shift) + gbase[b] + ((uint32_t)q - tstart[b])] = e;
+        const uint32_t b = __float_as_uint(e.w) >> shift, bl = b & lmask;
+        out[((size_t)b << shift) + gbase[bl] + ((uint32_t)q - tstart[bl])] = e;
       }
     }
     __syncthreads();
   }
-  (void)nbins;
 }
 
 template <bool kKick>
-__global__ void __launch_bounds__(256) k_unsort_apply(const float4* __restrict__ buf, int64_t n, float4* __restrict__ acc,
-                                                       float4* __restrict__ vel, float kdt) {
-  constexpr int U = 4;
-  for (int64_t k0 = (int64_t)blockIdx.x * blockDim.x * U + threadIdx.x; k0 < n; k0 += (int64_t)gridDim.x * blockDim.x * U) {
-    float4 e[U], v[U];
+__global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_final(const float4* __restrict__ buf, int64_t n,
+                                                                     float4* __restrict__ acc, float4* __restrict__ vel,
+                                                                     float kdt) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float4* stile = (float4*)smem_raw;                       // [kUnsortTile] destination order
+  const int64_t nwin = (n + kUnsortTile - 1) / kUnsortTile;
+  for (int64_t t = blockIdx.x; t < nwin; t += gridDim.x) {
+    const int64_t base = t * kUnsortTile;
+    const int win_n = (int)min((int64_t)kUnsortTile, n - base);
+    {
+      float4 e[kUnsortItems];
 #pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const int64_t k = k0 + (int64_t)u * blockDim.x;
-      if (k < n) {
-        e[u] = __ldcs(&buf[k]);
-        if (kKick) v[u] = vel[__float_as_uint(e[u].w)];
+      for (int u = 0; u < kUnsortItems; ++u) {
+        const int q = u * kUnsortThreads + threadIdx.x;
+        if (q < win_n) e[u] = __ldcs(&buf[base + q]);
       }
-    }
 #pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const int64_t k = k0 + (int64_t)u * blockDim.x;
-      if (k < n) {
-        const uint32_t dst = __float_as_uint(e[u].w);
-        acc[dst] = make_float4(e[u].x, e[u].y, e[u].z, 0.f);
-        if (kKick) {
-          v[u].x = __fmaf_rn(e[u].x, kdt, v[u].x); v[u].y = __fmaf_rn(e[u].y, kdt, v[u].y); v[u].z = __fmaf_rn(e[u].z, kdt, v[u].z);
-          vel[dst] = v[u];
+      for (int u = 0; u < kUnsortItems; ++u)
+        if (u * kUnsortThreads + (int)threadIdx.x < win_n) stile[__float_as_uint(e[u].w) & (kUnsortTile - 1)] = e[u];
+    }
+    __syncthreads();
+    // linear output, four elements per thread in flight (with the kick: their velocities too)
+#pragma unroll 1
+    for (int h = 0; h < kUnsortItems; h += 4) {
+      float4 v[4];
+      if (kKick) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int q = (h + u) * kUnsortThreads + threadIdx.x;
+          if (q < win_n) v[u] = vel[base + q];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int q = (h + u) * kUnsortThreads + threadIdx.x;
+        if (q < win_n) {
+          const float4 a = stile[q];
+          acc[base + q] = make_float4(a.x, a.y, a.z, 0.f);
+          if (kKick) {
+            v[u].x = __fmaf_rn(a.x, kdt, v[u].x); v[u].y = __fmaf_rn(a.y, kdt, v[u].y); v[u].z = __fmaf_rn(a.z, kdt, v[u].z);
+            vel[base + q] = v[u];
+          }
         }
       }
     }
+    __syncthreads();
   }
 }
 
@@ -636,27 +668,43 @@ cudaError_t launch_write_back(srpp_ctx* c, float4* acc, float4* vel, float kdt) 
     c->launches += 1;
     return cudaGetLastError();
   }
-  // buckets of 2^shift consecutive destinations, at most kUnsortMaxBins of them
-  int shift = 16;
-  while (((n + ((int64_t)1 << shift) - 1) >> shift) > kUnsortMaxBins) ++shift;
-  const int nbins = (int)((n + ((int64_t)1 << shift) - 1) >> shift);
-  float4* buf = c->sorted == c->sorted_buf[0] ? c->sorted_buf[1] : c->sorted_buf[0];   // the re-bin's idle ping-pong partner
+  // levels: the window index (destination >> 12) has `tb` bits, split evenly over the levels, <= 8 bits each
+  const int64_t nwin = (n + kUnsortTile - 1) >> kUnsortWinBits;
+  int tb = 1;
+  while (((int64_t)1 << tb) < nwin) ++tb;
+  const int nlev = (tb + 7) / 8;
+  const int o = c->sorted == c->sorted_buf[0] ? 1 : 0;            // the idle partners of the sub-cycle's ping-pong buffers
+  float4* bufs[2] = {c->sorted_buf[o], c->vel_s[o]};
   const size_t smem = (size_t)kUnsortTile * sizeof(float4) + (3 * kUnsortMaxBins + 32) * sizeof(uint32_t);
+  const size_t smem_fin = (size_t)kUnsortTile * sizeof(float4);
+  cudaError_t e;
   if (!c->unsort_attr_set) {
-    const cudaError_t ea = cudaFuncSetAttribute(k_unsort_partition, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (ea != cudaSuccess) return ea;
+    if ((e = cudaFuncSetAttribute(k_unsort_partition<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_unsort_partition<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_unsort_final<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_unsort_final<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fin)) != cudaSuccess) return e;
     c->unsort_attr_set = true;
   }
-  cudaError_t e;
-  if ((e = cudaMemsetAsync(c->unsort_cursor, 0, sizeof(uint32_t) * kUnsortMaxBins, st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(c->unsort_cursor, 0, unsort_cursor_bytes(n), st)) != cudaSuccess) return e;
   const int64_t ntiles = (n + kUnsortTile - 1) / kUnsortTile;
-  k_unsort_partition<<<(int)std::min<int64_t>(ntiles, (int64_t)c->num_sms * 2), kUnsortThreads, smem, st>>>(
-      c->acc64, c->perm, n, scale, shift, nbins, c->unsort_cursor, buf);
-  // few CTAs in flight keep the windows of scattered stores small (they have to stay in L2 until complete)
-  const int grid_ap = (int)std::min<int64_t>((n + 1023) / 1024, (int64_t)c->num_sms * 4);
-  if (vel) k_unsort_apply<true><<<grid_ap, 256, 0, st>>>(buf, n, acc, vel, kdt);
-  else k_unsort_apply<false><<<grid_ap, 256, 0, st>>>(buf, n, acc, nullptr, 0.f);
-  c->launches += 2;
+  const int grid = (int)std::min<int64_t>(ntiles, (int64_t)c->num_sms * 2);
+  int prev_shift = 31, bits_left = tb;
+  uint32_t* cursor = c->unsort_cursor;
+  const float4* in = nullptr;
+  for (int l = 0; l < nlev; ++l) {
+    const int bl = (bits_left + (nlev - l) - 1) / (nlev - l);      // bits of this level
+    bits_left -= bl;
+    const int shift = kUnsortWinBits + bits_left;
+    float4* out = bufs[l & 1];
+    if (l == 0) k_unsort_partition<true><<<grid, kUnsortThreads, smem, st>>>(c->acc64, c->perm, nullptr, n, scale, prev_shift, shift, cursor, out);
+    else k_unsort_partition<false><<<grid, kUnsortThreads, smem, st>>>(nullptr, nullptr, in, n, scale, prev_shift, shift, cursor, out);
+    cursor += ((n - 1) >> shift) + 1;                               // this level's buckets
+    prev_shift = shift;
+    in = out;
+  }
+  if (vel) k_unsort_final<true><<<grid, kUnsortThreads, smem_fin, st>>>(in, n, acc, vel, kdt);
+  else k_unsort_final<false><<<grid, kUnsortThreads, smem_fin, st>>>(in, n, acc, nullptr, 0.f);
+  c->launches += (uint64_t)nlev + 1;
   return cudaGetLastError();
 }
 

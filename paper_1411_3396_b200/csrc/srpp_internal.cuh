@@ -30,6 +30,8 @@ constexpr int kSrcTile = 128;                 // sources staged per warp-private
 constexpr int kSrcChunk = 1024;               // sources per work item (fp32 partial-sum length)
 constexpr int kMaxSeg = 18;                   // 9 (dy,dz) rows x up to 2 x-segments (periodic wrap)
 constexpr int64_t kUnsortMinN = (int64_t)1 << 22;   // write-back: below this acc and vel sit in L2 and the direct scatter wins
+// run cursors of the bucketed write-back: one per bucket of every level (at most 256 + 65536 + n/4096 + 3)
+constexpr size_t unsort_cursor_bytes(int64_t n) { return sizeof(uint32_t) * ((size_t)(n > 0 ? n : 1) / 4096 + 65536 + 256 + 8); }
 
 // timing events: mesh begin/end, accel begin, force-kernel begin/end, accel end
 enum { kEvMesh0 = 0, kEvMesh1, kEvAccel0, kEvForce0, kEvForce1, kEvAccel1, kNumEvents };
@@ -109,7 +111,7 @@ struct srpp_ctx {
   int sort_blocks_per_sm;
   bool sort_attr_set;
   bool unsort_attr_set;
-  uint32_t* unsort_cursor;   // [256] run cursors of the bucketed write-back (srpp_force.cu)
+  uint32_t* unsort_cursor;   // run cursors of the bucketed write-back (srpp_force.cu), unsort_cursor_bytes(n)
   bool uniform_mass;
   float mass0;
   // workspace carve-up (device pointers)
