@@ -466,9 +466,11 @@ constexpr int kUnsortWinBits = 12;                        // final windows: 4096
 constexpr int kUnsortItems = kUnsortTile / kUnsortThreads;
 constexpr int kUnsortMaxBins = 256;
 
-// kFromAcc: first level (reads the fp64 accumulators and perm); else reads the previous level's elements.
+// kSrc 0: first level, elements made from the fp64 accumulators (x scale) and perm; 1: first level, elements made from
+// the xyz of a sorted float4 array and perm (the sub-cycle's positions / velocities going back to the caller's order);
+// 2: a later level, reads the previous level's elements.
 // prev_shift: the input is already grouped in windows of 2^prev_shift destinations (31: the whole array).
-template <bool kFromAcc>
+template <int kSrc>
 __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_partition(
     const double* __restrict__ acc64, const uint32_t* __restrict__ perm, const float4* __restrict__ in, int64_t n,
     float scale, int prev_shift, int shift, uint32_t* __restrict__ cursor /*[n >> shift, +1], cleared*/,
@@ -497,12 +499,13 @@ __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_partition(
       v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
       if (e < tile_n) {
         const int64_t k = base + e;
-        if (kFromAcc) {
+        if (kSrc == 0) {
           const uint32_t dst = __ldcs(&perm[k]);
           v[u] = make_float4((float)(__ldcs(&acc64[3 * k + 0]) * s), (float)(__ldcs(&acc64[3 * k + 1]) * s),
                              (float)(__ldcs(&acc64[3 * k + 2]) * s), __uint_as_float(dst));
         } else {
           v[u] = __ldcs(&in[k]);
+          if (kSrc == 1) v[u].w = __uint_as_float(__ldcs(&perm[k]));
         }
       }
     }
@@ -541,10 +544,13 @@ __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_partition(
   }
 }
 
-template <bool kKick>
+// kMode 0: acc = (x, y, z, 0); 1: the same and the kick v <- fmaf(a, kdt, v) on vel; 2: xyz written into acc's elements,
+// their .w lanes kept (positions with their masses, velocities).
+template <int kMode>
 __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_final(const float4* __restrict__ buf, int64_t n,
                                                                      float4* __restrict__ acc, float4* __restrict__ vel,
                                                                      float kdt) {
+  constexpr bool kKick = kMode == 1;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* stile = (float4*)smem_raw;                       // [kUnsortTile] destination order
   const int64_t nwin = (n + kUnsortTile - 1) / kUnsortTile;
@@ -567,11 +573,11 @@ __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_final(const float4
 #pragma unroll 1
     for (int h = 0; h < kUnsortItems; h += 4) {
       float4 v[4];
-      if (kKick) {
+      if (kMode != 0) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const int q = (h + u) * kUnsortThreads + threadIdx.x;
-          if (q < win_n) v[u] = vel[base + q];
+          if (q < win_n) v[u] = kKick ? vel[base + q] : acc[base + q];
         }
       }
 #pragma unroll
@@ -579,7 +585,7 @@ __global__ void __launch_bounds__(kUnsortThreads, 2) k_unsort_final(const float4
         const int q = (h + u) * kUnsortThreads + threadIdx.x;
         if (q < win_n) {
           const float4 a = stile[q];
-          acc[base + q] = make_float4(a.x, a.y, a.z, 0.f);
+          acc[base + q] = make_float4(a.x, a.y, a.z, kMode == 2 ? v[u].w : 0.f);
           if (kKick) {
             v[u].x = __fmaf_rn(a.x, kdt, v[u].x); v[u].y = __fmaf_rn(a.y, kdt, v[u].y); v[u].z = __fmaf_rn(a.z, kdt, v[u].z);
             vel[base + q] = v[u];
@@ -656,18 +662,11 @@ cudaError_t launch_accel_sorted(srpp_ctx* c) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_write_back(srpp_ctx* c, float4* acc, float4* vel, float kdt) {
+// Bucketed un-sort of one array (n >= kUnsortMinN): `sorted_src` == nullptr takes the fp64 accumulators (A6), else
+// the xyz of a sorted float4 array; mode as in k_unsort_final.
+static cudaError_t launch_unsort(srpp_ctx* c, const float4* sorted_src, float scale, int mode, float4* dst, float4* vel, float kdt) {
   const int64_t n = c->n;
-  if (n == 0) return cudaSuccess;
   cudaStream_t st = c->stream;
-  const float scale = c->uniform_mass ? c->mass0 : 1.0f;
-  if (n < kUnsortMinN) {
-    const int grid_wb = (int)std::min<int64_t>((n + 1023) / 1024, (int64_t)c->num_sms * 16);
-    if (vel) k_write_back<true><<<grid_wb, 256, 0, st>>>(c->acc64, c->perm, n, scale, acc, vel, kdt);
-    else k_write_back<false><<<grid_wb, 256, 0, st>>>(c->acc64, c->perm, n, scale, acc, nullptr, 0.f);
-    c->launches += 1;
-    return cudaGetLastError();
-  }
   // levels: the window index (destination >> 12) has `tb` bits, split evenly over the levels, <= 8 bits each
   const int64_t nwin = (n + kUnsortTile - 1) >> kUnsortWinBits;
   int tb = 1;
@@ -679,10 +678,12 @@ cudaError_t launch_write_back(srpp_ctx* c, float4* acc, float4* vel, float kdt) 
   const size_t smem_fin = (size_t)kUnsortTile * sizeof(float4);
   cudaError_t e;
   if (!c->unsort_attr_set) {
-    if ((e = cudaFuncSetAttribute(k_unsort_partition<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_unsort_partition<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_unsort_final<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fin)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_unsort_final<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_unsort_partition<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_unsort_partition<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_unsort_partition<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_unsort_final<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_unsort_final<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fin)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_unsort_final<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fin)) != cudaSuccess) return e;
     c->unsort_attr_set = true;
   }
   if ((e = cudaMemsetAsync(c->unsort_cursor, 0, unsort_cursor_bytes(n), st)) != cudaSuccess) return e;
@@ -696,16 +697,38 @@ cudaError_t launch_write_back(srpp_ctx* c, float4* acc, float4* vel, float kdt) 
     bits_left -= bl;
     const int shift = kUnsortWinBits + bits_left;
     float4* out = bufs[l & 1];
-    if (l == 0) k_unsort_partition<true><<<grid, kUnsortThreads, smem, st>>>(c->acc64, c->perm, nullptr, n, scale, prev_shift, shift, cursor, out);
-    else k_unsort_partition<false><<<grid, kUnsortThreads, smem, st>>>(nullptr, nullptr, in, n, scale, prev_shift, shift, cursor, out);
+    if (l == 0 && !sorted_src) k_unsort_partition<0><<<grid, kUnsortThreads, smem, st>>>(c->acc64, c->perm, nullptr, n, scale, prev_shift, shift, cursor, out);
+    else if (l == 0) k_unsort_partition<1><<<grid, kUnsortThreads, smem, st>>>(nullptr, c->perm, sorted_src, n, 1.f, prev_shift, shift, cursor, out);
+    else k_unsort_partition<2><<<grid, kUnsortThreads, smem, st>>>(nullptr, nullptr, in, n, 1.f, prev_shift, shift, cursor, out);
     cursor += ((n - 1) >> shift) + 1;                               // this level's buckets
     prev_shift = shift;
     in = out;
   }
-  if (vel) k_unsort_final<true><<<grid, kUnsortThreads, smem_fin, st>>>(in, n, acc, vel, kdt);
-  else k_unsort_final<false><<<grid, kUnsortThreads, smem_fin, st>>>(in, n, acc, nullptr, 0.f);
+  if (mode == 1) k_unsort_final<1><<<grid, kUnsortThreads, smem_fin, st>>>(in, n, dst, vel, kdt);
+  else if (mode == 2) k_unsort_final<2><<<grid, kUnsortThreads, smem_fin, st>>>(in, n, dst, nullptr, 0.f);
+  else k_unsort_final<0><<<grid, kUnsortThreads, smem_fin, st>>>(in, n, dst, nullptr, 0.f);
   c->launches += (uint64_t)nlev + 1;
   return cudaGetLastError();
+}
+
+cudaError_t launch_write_back(srpp_ctx* c, float4* acc, float4* vel, float kdt) {
+  const int64_t n = c->n;
+  if (n == 0) return cudaSuccess;
+  cudaStream_t st = c->stream;
+  const float scale = c->uniform_mass ? c->mass0 : 1.0f;
+  if (n < kUnsortMinN) {
+    const int grid_wb = (int)std::min<int64_t>((n + 1023) / 1024, (int64_t)c->num_sms * 16);
+    if (vel) k_write_back<true><<<grid_wb, 256, 0, st>>>(c->acc64, c->perm, n, scale, acc, vel, kdt);
+    else k_write_back<false><<<grid_wb, 256, 0, st>>>(c->acc64, c->perm, n, scale, acc, nullptr, 0.f);
+    c->launches += 1;
+    return cudaGetLastError();
+  }
+  return launch_unsort(c, nullptr, scale, vel ? 1 : 0, acc, vel, kdt);
+}
+
+// xyz of a sorted array back into the caller's array (its .w lanes are kept); n >= kUnsortMinN only
+cudaError_t launch_unsort_xyz(srpp_ctx* c, const float4* sorted_src, float4* dst) {
+  return launch_unsort(c, sorted_src, 1.f, 2, dst, nullptr, 0.f);
 }
 
 cudaError_t launch_accel(srpp_ctx* c, float4* acc, float4* vel, float kdt) {

@@ -187,6 +187,7 @@ void plan_sort(int32_t ncells, int* passes, int* digit_bits);
 cudaError_t launch_accel(srpp_ctx* c, float4* acc, float4* vel = nullptr, float kdt = 0.f);
 cudaError_t launch_accel_sorted(srpp_ctx* c);                  // force only: fp64 accumulators in sorted order
 cudaError_t launch_write_back(srpp_ctx* c, float4* acc, float4* vel = nullptr, float kdt = 0.f);   // A6 (+ A7)
+cudaError_t launch_unsort_xyz(srpp_ctx* c, const float4* sorted_src, float4* dst);   // bucketed scatter of xyz through perm
 // srpp_subcycle.cu
 cudaError_t launch_subcycle(srpp_ctx* c, float4* pos_mass, float4* vel, float4* acc, float dt, float kdt, int nsub,
                             int64_t n, int32_t* status_out);

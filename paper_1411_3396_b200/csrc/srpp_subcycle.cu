@@ -236,6 +236,13 @@ static inline int ew_grid(const srpp_ctx* c, int64_t n) { return (int)std::min<i
 // scatter the sorted state back to the caller's order
 static cudaError_t unsort_state(srpp_ctx* c, int cur, float4* pos_mass, float4* vel, int64_t n) {
   if (n == 0) return cudaSuccess;
+  if (n >= kUnsortMinN) {
+    // large n: the destinations have no locality; partition by destination instead of scattering (srpp_force.cu A6).
+    // Only xyz travel: the caller's arrays still hold the masses / the velocities' .w lanes, which no step changes.
+    cudaError_t e = launch_unsort_xyz(c, c->sorted_buf[cur], pos_mass);
+    if (e == cudaSuccess) e = launch_unsort_xyz(c, c->vel_s[cur], vel);
+    return e;
+  }
   k_scatter2_f4<<<ew_grid(c, n), 256, 0, c->stream>>>(c->sorted_buf[cur], c->vel_s[cur], c->perm, n, pos_mass, vel);
   c->launches += 1;
   return cudaGetLastError();

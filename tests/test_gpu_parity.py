@@ -430,6 +430,44 @@ def test_subcycle_step_by_step(oracle_mod, gpu):
         x0, v0 = x1, v1
 
 
+def test_subcycle_large_n_bucketed_paths(oracle_mod, gpu):
+    """srpp_subcycle above 2^22 particles: the write-back and the return of positions and velocities to the caller's
+    order take the bucketed (partition by destination) path, with a ragged last tile and window; unequal masses and
+    non-zero velocity .w lanes must come back untouched.  Same checks as the step-by-step test, one sub-step."""
+    torch, binding = gpu
+    n, ncell = (1 << 22) + 4099, (50, 50, 51)
+    rng = np.random.default_rng(9)
+    box = tuple(3.2 * c for c in ncell)
+    pos = np.empty((n, 4), dtype=np.float32)
+    pos[:, :3] = (rng.random((n, 3)) * np.asarray(box)).astype(np.float32)
+    pos[:, :3] = np.minimum(pos[:, :3], np.nextafter(np.asarray(box, dtype=np.float32), 0))
+    pos[:, 3] = rng.uniform(0.5, 2.0, n).astype(np.float32)
+    vel = rng.normal(0, 1.0, (n, 4)).astype(np.float32)
+    sol = binding.Solver(box, ncell, 3.0, 0.1, n_max=n)
+    d_pos, d_vel = torch.from_numpy(pos.copy()).cuda(), torch.from_numpy(vel.copy()).cuda()
+    dt, kdt = 0.05, 0.04
+    acc = sol.subcycle(d_pos, d_vel, dt, kdt, 1)
+    torch.cuda.synchronize()
+    a, x1, v1 = acc.cpu().numpy(), d_pos.cpu().numpy(), d_vel.cpu().numpy()
+    half = np.float32(0.5) * np.float32(dt)
+    x_mid = oracle_mod.stream(pos, vel, half, box)
+    ref, st = oracle_mod.accel(x_mid, oracle_mod.make_params(box, 3.0, 0.1), stats=True)
+    per, glob = oracle_mod.error_norms(a, ref, st["allowance"])
+    assert per.max() <= PER_PARTICLE_TOL and glob <= GLOBAL_L2_TOL, (per.max(), glob)
+    v_exp = oracle_mod.kick(vel, a, kdt)
+    assert np.array_equal(v1.view(np.uint32), v_exp.view(np.uint32))          # incl. the .w lanes
+    x_exp = oracle_mod.stream(x_mid, v_exp, half, box)
+    assert np.array_equal(x1.view(np.uint32), x_exp.view(np.uint32))          # incl. the masses
+    cs, perm, srt = (t.cpu().numpy() for t in sol.get_mesh())
+    o_cs, o_perm, o_srt = oracle_mod.build_mesh(x1, box, ncell)
+    assert np.array_equal(cs.view(np.uint32), o_cs) and np.array_equal(perm.view(np.uint32), o_perm)
+    assert np.array_equal(srt.view(np.uint32), o_srt.view(np.uint32))
+    stt = sol.get_stats()
+    moved = np.mean(oracle_mod.cell_ids(pos, box, ncell) != oracle_mod.cell_ids(x1, box, ncell))
+    print("large-n sub-step: %.2f %% changed cell, re-bins incremental %d full %d; accel per-particle %.2e, L2 %.2e"
+          % (100 * moved, stt["rebins_incremental"], stt["rebins_full"], per.max(), glob))
+
+
 def test_subcycle_several_substeps_vs_oracle(oracle_mod, gpu):
     """nsub = 4 in one call against orc_subcycle from the same start: the trajectories differ only by the fp32-vs-fp64
     rounding of the accelerations (1e-6 relative), far below the per-step changes."""
