@@ -64,7 +64,7 @@ __device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint
   return s;
 }
 
-// Targets of one work item.  Large cells: 32 lanes x 4 targets (two packed pairs per lane), several items per cell.
+// Targets of one work item.  Large cells: 32 lanes x 6 targets (three packed pairs per lane), several items per cell.
 // Cells of <= 48 particles (the uniform background: ~33 per cell) would leave half of a 64-target tile empty, so
 // there the warp is split over the SOURCES: with S source phases, 32/S lanes x 2 targets = 64/S targets per packed
 // pair, TP packed pairs per lane cover the WHOLE cell in one item (the staged sources are shared by all its targets),
@@ -72,12 +72,13 @@ __device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint
 // with shuffles at the end.  Cells of <= 40 particles use S = 8 (targets padded to a multiple of 8: 1.10 pair slots
 // per candidate pair at ~33 per cell; S = 4 with its multiples of 16 gave 1.23), 41..48 use S = 4 (48 slots), 49..64
 // take one 64-target item.
+constexpr int kBigTP = 3;                       // packed target pairs per lane of a large-cell item (192 targets per item)
 constexpr uint32_t kSplit8MaxCell = 40;         // <= 5 packed pairs of 8 targets
 constexpr uint32_t kSplitMaxCell = 48;          // <= 3 packed pairs of 16 targets
 __device__ __forceinline__ uint32_t targets_per_item(uint32_t n_c, int fine) {
   if (n_c <= kSplit8MaxCell) return fine ? min(16u, ((n_c + 7u) / 8u) * 8u) : ((n_c + 7u) / 8u) * 8u;   // fine: tiny problems need more items
   if (n_c <= kSplitMaxCell) return fine ? 16u : 48u;
-  return n_c <= 64u ? 64u : 128u;
+  return n_c <= 64u ? 64u : 64u * (uint32_t)kBigTP;
 }
 
 // ------------------------------------------------------------------- plan: items per cell, W, max --
@@ -257,10 +258,13 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
     __syncwarp();
     // ---- pair loop: every source of the tile against the lane's 2*TP targets
     const int cnt = (int)min((uint32_t)kSrcTile, (p1 - tile + (uint32_t)(S - 1)) & ~(uint32_t)(S - 1));
-    // unrolled to about 8 packed-pair bodies per trip: the variants run side by side on one SM sub-partition (cells of
-    // 20..46 particles pick four of them), and bodies of 20 packed pairs each (7 KB of code per variant) thrashed the
-    // instruction cache -- FMA-pipe utilisation fell from 83 % to 63 %
-#pragma unroll (TP >= 3 ? 2 : 4)
+    // Small-cell variants (S > 1) are unrolled to about 8 packed-pair bodies per trip: they run side by side on one SM
+    // sub-partition (cells of 20..46 particles pick four of them), and bodies of 20 packed pairs each (7 KB of code per
+    // variant) thrashed the instruction cache -- FMA-pipe utilisation fell from 83 % to 63 %.  The large-cell variant is
+    // alone on the chip for most of its time: 16 sources x 3 packed pairs per trip gives ptxas the freedom to keep the
+    // FMA pipe fed across the MUFU latencies (measured on config 3: TP 2 / unroll 4 71.3 %, TP 3 / unroll 4 72.7 %,
+    // TP 3 / unroll 8 73.5 %, TP 3 / unroll 16 73.9 %, TP 3 / unroll 32 73.5 %, TP 4 / unroll 8 72.4 % of FP32 peak).
+#pragma unroll (S > 1 ? (TP >= 3 ? 2 : 4) : 16)
     for (int j = (S > 1 ? lane / (32 / S) : 0); j < cnt; j += S) {
       // one LDS.128 per source; the packed instructions broadcast the scalar to both halves (R.F32 operand form)
       const float4 sv = ws.src[j];
@@ -406,7 +410,7 @@ k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_
     else if (n_c <= 64u)
       process_item<1, kUniformMass, 1>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
     else
-      process_item<2, kUniformMass, 1>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
+      process_item<kBigTP, kUniformMass, 1>(ws, sorted, fc, tb, te, ref_t, p0, p1, acc64, lane, lane_zero);
   }
 }
 

@@ -26,8 +26,14 @@ constexpr size_t sort_ctl_bytes() { return sizeof(uint32_t) * (64 + (size_t)kSor
 
 constexpr int kForceThreads = 256;            // 8 autonomous warps per CTA
 constexpr int kForceWarps = kForceThreads / 32;
-constexpr int kSrcTile = 128;                 // sources staged per warp-private smem tile (float4 each)
-constexpr int kSrcChunk = 1024;               // sources per work item (fp32 partial-sum length)
+#ifndef SRPP_SRC_TILE
+#define SRPP_SRC_TILE 128
+#endif
+#ifndef SRPP_SRC_CHUNK
+#define SRPP_SRC_CHUNK 1024
+#endif
+constexpr int kSrcTile = SRPP_SRC_TILE;       // sources staged per warp-private smem tile (float4 each)
+constexpr int kSrcChunk = SRPP_SRC_CHUNK;     // sources per work item (fp32 partial-sum length)
 constexpr int kMaxSeg = 18;                   // 9 (dy,dz) rows x up to 2 x-segments (periodic wrap)
 constexpr int64_t kUnsortMinN = (int64_t)1 << 22;   // write-back: below this acc and vel sit in L2 and the direct scatter wins
 // run cursors of the bucketed write-back: one per bucket of every level (at most 256 + 65536 + n/4096 + 3)

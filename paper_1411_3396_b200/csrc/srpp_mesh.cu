@@ -12,13 +12,15 @@
 //   k_sort_prepass   one read of the positions: domain / mass flags (R13, R14) and the GLOBAL histogram of every digit
 //                    (A2; <= 3 x 256 counters).  The cell id is never stored: each pass recomputes it from the
 //                    position it carries (3 multiplies + floor, far below the memory time).
-//   k_sort_pass      per digit: CTAs take tiles of 4096 consecutive elements in ticket order, every thread holding 4
-//                    elements in registers (requested one tile ahead); stable ranks come from per-warp {peer mask,
+//   k_sort_pass      per digit: two CTAs of 512 threads per SM take tiles of 4096 consecutive elements in ticket order,
+//                    every thread holding 8 elements in registers (requested one tile ahead; the tile gridDim.x
+//                    tickets ahead is pulled into L2 by a TMA prefetch); stable ranks come from per-warp {peer mask,
 //                    running count} tables in warp-major order (no atomic decides a position, so perm is
 //                    reproducible and equals the oracle's stable counting sort); the exclusive prefix of every digit
 //                    over the earlier tiles comes from a decoupled look-back over per-tile status words (A3:
 //                    aggregate published right after the tile histogram, inclusive prefix after the look-back); the
-//                    tile is re-ordered by digit in shared memory and written out as per-digit runs.
+//                    tile is re-ordered by digit in shared memory and leaves as per-digit runs -- TMA bulk stores, one
+//                    per digit thread, in every pass but the last (equal masses), ordinary stores otherwise.
 //                    Equal masses (every BASELINE.json config): the original index travels in the .w lane of the
 //                    position (16 bytes per element and pass) and the mass is restored by the last pass; otherwise it
 //                    travels in a separate array (20 bytes).  The last pass also writes perm and the sorted cell ids.
@@ -181,9 +183,13 @@ constexpr uint32_t kStatAgg = 1u, kStatPrefix = 2u;
 #ifndef SRPP_LOOK_WINDOW
 #define SRPP_LOOK_WINDOW 4
 #endif
-constexpr int kPassThreads = SRPP_PASS_THREADS;         // 32 warps, one CTA per SM: the pass is bound by shared-memory
-constexpr int kPassWarps = kPassThreads / 32;           // wavefronts and the latency between its phases, not by DRAM
-constexpr int kPassItems = kPassTile / kPassThreads;    // (2 CTAs x 512 threads x 2048-element tiles measured slower)
+// Two CTAs of 512 threads per SM, 8 elements per thread: a pass is bound by issue slots, shared-memory wavefronts and
+// the barrier-separated phases of a tile, not by DRAM, and the second CTA fills the first one's barrier waits
+// (measured on config 4: 1024 threads x 1 CTA 1.38 ms per build, 512 x 2 1.25 ms; tiles of 2048 elements are slower:
+// shorter per-digit runs).  The tunables can be overridden with -D for experiments.
+constexpr int kPassThreads = SRPP_PASS_THREADS;
+constexpr int kPassWarps = kPassThreads / 32;
+constexpr int kPassItems = kPassTile / kPassThreads;
 constexpr int kPassCtasPerSm = SRPP_PASS_CTAS;
 constexpr int kLookWindow = SRPP_LOOK_WINDOW;                          // status words of earlier tiles read per round trip
 
@@ -198,9 +204,9 @@ __host__ __device__ inline size_t sort_pass_smem(int nbins, bool packed) {
 }
 
 // One digit pass.  Per tile of 4096 consecutive elements (ticket order):
-//   * every thread holds 4 elements of the tile in registers (warp w owns the 128 consecutive elements
-//     [128 w, 128 w + 128) in 4 steps of 32, so (tile, warp, step, lane) order == input order); they were requested
-//     while the previous tile was written out;
+//   * every thread holds kPassItems (8) elements of the tile in registers (warp w owns the 256 consecutive elements
+//     [256 w, 256 w + 256) in 8 steps of 32, so (tile, warp, step, lane) order == input order); they were requested
+//     as soon as the previous tile had left the registers;
 //   * stable ranks, no atomic decides a position: per step the lanes holding the same digit find each other through a
 //     per-warp table -- every lane ORs its lane bit into the mask of its digit, reads mask and running count back
 //     (rank = count + number of lower peers), and the lowest peer clears the mask and advances the count.  Which
