@@ -156,7 +156,7 @@ int32_t srpp_create(srpp_ctx** out, const srpp_params* params, void* workspace, 
   cudaError_t e = cudaGetDevice(&c->device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
   if (e != cudaSuccess) { delete c; return SRPP_ERR_CUDA; }
-  c->force_blocks_per_sm = query_force_occupancy();
+  query_force_occupancy(c->force_blocks_per_sm);
 
   Geometry& g = c->geo;
   int64_t ncells = 1;

@@ -64,7 +64,7 @@ __device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint
   return s;
 }
 
-// Targets of one work item.  Large cells: 32 lanes x 6 targets (three packed pairs per lane), several items per cell.
+// Targets of one work item.  Large cells: 32 lanes x 8 targets (four packed pairs per lane), several items per cell.
 // Cells of <= 48 particles (the uniform background: ~33 per cell) would leave half of a 64-target tile empty, so
 // there the warp is split over the SOURCES: with S source phases, 32/S lanes x 2 targets = 64/S targets per packed
 // pair, TP packed pairs per lane cover the WHOLE cell in one item (the staged sources are shared by all its targets),
@@ -72,7 +72,19 @@ __device__ __forceinline__ Segment stencil_segment(const Geometry& g, const uint
 // with shuffles at the end.  Cells of <= 40 particles use S = 8 (targets padded to a multiple of 8: 1.10 pair slots
 // per candidate pair at ~33 per cell; S = 4 with its multiples of 16 gave 1.23), 41..48 use S = 4 (48 slots), 49..64
 // take one 64-target item.
-constexpr int kBigTP = 3;                       // packed target pairs per lane of a large-cell item (192 targets per item)
+// Two builds of the force kernel; the plan kernel decides on the device which one runs (the other returns at once):
+//   build 0 (most of W in cells of <= 64 particles: the uniform background, configs 1-2): CTAs of 8 warps, 2 per SM
+//            = 16 warps with <= 128 registers -- the small-cell items are short and latency-bound, more warps win
+//            (config 2: 55.9 % of FP32 peak against 53.6 % with build 1);
+//   build 1 (most of W in large cells: every clustered config): CTAs of 4 warps, 3 per SM = 12 warps with <= 168
+//            registers, which the large-cell item needs for its 4 packed target pairs per lane (256 targets) and 8
+//            sources per trip (config 3: 74.8 % of FP32 peak; with 128 registers the best form is 3 pairs x 16 sources
+//            at 73.9 %, 4 pairs x 8 sources 72.4 %; 8 warps per SM with 212 / 251 registers and 6 / 8 pairs: 73.0 / 72.9 %).
+// The work plan (items per cell) is the same for both: large-cell items hold kBigTP packed pairs per lane.
+template <int kBuild> struct PPBuild;
+template <> struct PPBuild<0> { static constexpr int kThreads = 256, kCtasPerSm = 2; };
+template <> struct PPBuild<1> { static constexpr int kThreads = 128, kCtasPerSm = 3; };
+constexpr int kBigTP = 4;                       // packed target pairs per lane of a large-cell item (256 targets per item)
 constexpr uint32_t kSplit8MaxCell = 40;         // <= 5 packed pairs of 8 targets
 constexpr uint32_t kSplitMaxCell = 48;          // <= 3 packed pairs of 16 targets
 __device__ __forceinline__ uint32_t targets_per_item(uint32_t n_c, int fine) {
@@ -85,7 +97,7 @@ __device__ __forceinline__ uint32_t targets_per_item(uint32_t n_c, int fine) {
 __global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__ cell_start, Geometry g, int fine,
                                                      unsigned long long* __restrict__ items, DevFlags* flags) {
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  unsigned long long w = 0, slots = 0;
+  unsigned long long w = 0, slots = 0, wbig = 0;
   uint32_t nmax = 0;
   if (c < g.ncells) {
     const uint32_t n_c = __ldg(&cell_start[c + 1]) - __ldg(&cell_start[c]);
@@ -104,6 +116,7 @@ __global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__
       const unsigned long long nchunk = (S + kSrcChunk - 1) / kSrcChunk;
       it = ntile * nchunk;
       w = (unsigned long long)n_c * S;
+      wbig = n_c > 64u ? w : 0ull;
       const unsigned long long sp = (n_c <= kSplit8MaxCell || (fine && n_c <= kSplitMaxCell)) ? 7ull : (n_c <= kSplitMaxCell ? 3ull : 0ull);
       slots = ntile * tpi * ((S + sp) & ~sp);
       nmax = n_c;
@@ -114,11 +127,13 @@ __global__ void __launch_bounds__(256) k_plan_items(const uint32_t* __restrict__
   for (int o = 16; o; o >>= 1) {
     w += __shfl_xor_sync(0xffffffffu, w, o);
     slots += __shfl_xor_sync(0xffffffffu, slots, o);
+    wbig += __shfl_xor_sync(0xffffffffu, wbig, o);
     nmax = max(nmax, __shfl_xor_sync(0xffffffffu, nmax, o));
   }
   if ((threadIdx.x & 31) == 0) {
     if (w) atomicAdd(&flags->candidate_pairs, w);
     if (slots) atomicAdd(&flags->pair_slots, slots);
+    if (wbig) atomicAdd(&flags->big_pairs, wbig);
     if (nmax) atomicMax(&flags->max_cell_count, nmax);
   }
 }
@@ -261,10 +276,11 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
     // Small-cell variants (S > 1) are unrolled to about 8 packed-pair bodies per trip: they run side by side on one SM
     // sub-partition (cells of 20..46 particles pick four of them), and bodies of 20 packed pairs each (7 KB of code per
     // variant) thrashed the instruction cache -- FMA-pipe utilisation fell from 83 % to 63 %.  The large-cell variant is
-    // alone on the chip for most of its time: 16 sources x 3 packed pairs per trip gives ptxas the freedom to keep the
-    // FMA pipe fed across the MUFU latencies (measured on config 3: TP 2 / unroll 4 71.3 %, TP 3 / unroll 4 72.7 %,
-    // TP 3 / unroll 8 73.5 %, TP 3 / unroll 16 73.9 %, TP 3 / unroll 32 73.5 %, TP 4 / unroll 8 72.4 % of FP32 peak).
-#pragma unroll (S > 1 ? (TP >= 3 ? 2 : 4) : 16)
+    // alone on the chip for most of its time: 8 sources x 4 packed pairs per trip gives ptxas the freedom to keep the
+    // FMA pipe fed across the MUFU latencies (measured on config 3 at 128 registers: TP 2 / unroll 4 71.3 %, TP 3 /
+    // unroll 4 72.7 %, TP 3 / unroll 16 73.9 %, TP 3 / unroll 32 73.5 %; at 168 registers: TP 4 / unroll 8 74.8 %,
+    // TP 4 / unroll 12 74.3 %, TP 5 / unroll 8 72.3 % of FP32 peak).
+#pragma unroll (S > 1 ? (TP >= 3 ? 2 : 4) : 8)
     for (int j = (S > 1 ? lane / (32 / S) : 0); j < cnt; j += S) {
       // one LDS.128 per source; the packed instructions broadcast the scalar to both halves (R.F32 operand form)
       const float4 sv = ws.src[j];
@@ -325,12 +341,14 @@ __device__ __forceinline__ void process_item(WarpScratch& ws, const float4* __re
   }
 }
 
-template <bool kUniformMass>
-__global__ void __launch_bounds__(kForceThreads, 2)
+template <bool kUniformMass, int kBuild>
+__global__ void __launch_bounds__(PPBuild<kBuild>::kThreads, PPBuild<kBuild>::kCtasPerSm)
 k_pp_force(const float4* __restrict__ sorted, const uint32_t* __restrict__ cell_start,
            const unsigned long long* __restrict__ item_prefix, Geometry g, ForceConst fc, DevFlags* flags,
            double* __restrict__ acc64) {
-  __shared__ WarpScratch scratch[kForceWarps];
+  // the build is a device-side fact (found by the plan kernel): both are launched, one returns at once
+  if ((2ull * flags->big_pairs > flags->candidate_pairs ? 1 : 0) != kBuild) return;
+  __shared__ WarpScratch scratch[PPBuild<kBuild>::kThreads / 32];
   const int lane = threadIdx.x & 31;
   WarpScratch& ws = scratch[threadIdx.x >> 5];
   const unsigned long long total = flags->total_items;
@@ -626,12 +644,16 @@ __global__ void __launch_bounds__(256) k_stream(float4* __restrict__ pos, const 
 }
 
 // ------------------------------------------------------------------------------------ host launchers --
-int query_force_occupancy() {
+void query_force_occupancy(int* blocks_per_sm /*[2]*/) {
   int a = 0, b = 0;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k_pp_force<true>, kForceThreads, 0);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_pp_force<false>, kForceThreads, 0);
-  const int m = a < b ? a : b;
-  return m < 1 ? 1 : m;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k_pp_force<true, 0>, PPBuild<0>::kThreads, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_pp_force<false, 0>, PPBuild<0>::kThreads, 0);
+  blocks_per_sm[0] = a < b ? a : b;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k_pp_force<true, 1>, PPBuild<1>::kThreads, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_pp_force<false, 1>, PPBuild<1>::kThreads, 0);
+  blocks_per_sm[1] = a < b ? a : b;
+  for (int k = 0; k < 2; ++k)
+    if (blocks_per_sm[k] < 1) blocks_per_sm[k] = 1;
 }
 
 cudaError_t launch_scan_u64(cudaStream_t st, unsigned long long* data, int n, unsigned long long* tmp,
@@ -652,17 +674,21 @@ cudaError_t launch_accel_sorted(srpp_ctx* c) {
   // reset queue head + statistics (keep the binning flags)
   if ((e = cudaMemsetAsync(&c->flags->max_cell_count, 0, sizeof(DevFlags) - offsetof(DevFlags, max_cell_count), st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(c->acc64, 0, sizeof(double) * 3 * (size_t)n, st)) != cudaSuccess) return e;
-  c->fc.fine_items = n < (int64_t)c->num_sms * c->force_blocks_per_sm * kForceWarps * 64 ? 1 : 0;   // < 64 particles per resident warp
+  // fewer than 64 particles per resident warp (of build 0, the one tiny problems take): finer items
+  c->fc.fine_items = n < (int64_t)c->num_sms * c->force_blocks_per_sm[0] * (PPBuild<0>::kThreads / 32) * 64 ? 1 : 0;
   k_plan_items<<<(ncells + 255) / 256, 256, 0, st>>>(c->cell_start, c->geo, c->fc.fine_items, c->item_prefix, c->flags);
   if ((e = launch_scan_u64(st, c->item_prefix, ncells, c->scan_tmp, &c->flags->total_items, &c->item_prefix[ncells])) != cudaSuccess) return e;
-  const int grid = c->num_sms * c->force_blocks_per_sm;
+  const int grid0 = c->num_sms * c->force_blocks_per_sm[0], grid1 = c->num_sms * c->force_blocks_per_sm[1];
   if (c->timing) cudaEventRecord(c->ev[kEvForce0], st);
-  if (c->uniform_mass)
-    k_pp_force<true><<<grid, kForceThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
-  else
-    k_pp_force<false><<<grid, kForceThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
+  if (c->uniform_mass) {
+    k_pp_force<true, 0><<<grid0, PPBuild<0>::kThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
+    k_pp_force<true, 1><<<grid1, PPBuild<1>::kThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
+  } else {
+    k_pp_force<false, 0><<<grid0, PPBuild<0>::kThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
+    k_pp_force<false, 1><<<grid1, PPBuild<1>::kThreads, 0, st>>>(c->sorted, c->cell_start, c->item_prefix, c->geo, c->fc, c->flags, c->acc64);
+  }
   if (c->timing) cudaEventRecord(c->ev[kEvForce1], st);
-  c->launches += 5;
+  c->launches += 6;
   return cudaGetLastError();
 }
 

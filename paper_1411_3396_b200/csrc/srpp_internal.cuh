@@ -24,7 +24,10 @@ constexpr int kSortMaxPasses = 3;             // 3 x 8 bits cover the 2^24-cell 
 // sort control block: 64 words of tile tickets (one per pass) + the global digit histograms [passes][kSortMaxBins]
 constexpr size_t sort_ctl_bytes() { return sizeof(uint32_t) * (64 + (size_t)kSortMaxPasses * kSortMaxBins); }
 
-constexpr int kForceThreads = 256;            // 8 autonomous warps per CTA
+#ifndef SRPP_FORCE_THREADS
+#define SRPP_FORCE_THREADS 256
+#endif
+constexpr int kForceThreads = SRPP_FORCE_THREADS;   // 8 autonomous warps per CTA
 constexpr int kForceWarps = kForceThreads / 32;
 #ifndef SRPP_SRC_TILE
 #define SRPP_SRC_TILE 128
@@ -52,6 +55,7 @@ struct DevFlags {
   unsigned long long total_items;
   unsigned long long candidate_pairs; // W
   unsigned long long pair_slots;
+  unsigned long long big_pairs;       // part of W that sits in cells of more than 64 particles (picks the force kernel build)
 };
 
 struct Geometry {
@@ -108,7 +112,7 @@ struct srpp_ctx {
   cudaStream_t stream;
   int device;
   int num_sms;
-  int force_blocks_per_sm;
+  int force_blocks_per_sm[2];   // resident CTAs per SM of the two builds of the force kernel
   int64_t n_capacity;        // particles the workspace was sized for (== n of build_mesh)
   int64_t n;                 // particles of the last successful build_mesh, -1 before
   int sort_passes;           // digits of the cell id (LSD passes)
@@ -199,7 +203,7 @@ cudaError_t launch_subcycle(srpp_ctx* c, float4* pos_mass, float4* vel, float4* 
                             int64_t n, int32_t* status_out);
 cudaError_t launch_kick(srpp_ctx* c, float4* vel, const float4* acc, float kdt, int64_t n);
 cudaError_t launch_stream(srpp_ctx* c, float4* pos_mass, const float4* vel, float dt, int64_t n);
-int query_force_occupancy();
+void query_force_occupancy(int* blocks_per_sm /*[2]*/);
 // in-place exclusive scan of data[0..n) (n <= 2^24); the total goes to *total_out and *total_out2 (device pointers)
 cudaError_t launch_scan_u64(cudaStream_t st, unsigned long long* data, int n, unsigned long long* tmp,
                             unsigned long long* total_out, unsigned long long* total_out2);
