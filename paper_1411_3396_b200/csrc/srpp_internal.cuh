@@ -16,7 +16,10 @@ constexpr int kSortThreads = 512;             // 16 warps
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortItems = 8;                 // a warp handles 8 steps of 32 consecutive elements
 constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 elements per tile
-constexpr int kPassTile = 4096;               // elements per tile of a digit pass (k_sort_pass)
+#ifndef SRPP_PASS_TILE
+#define SRPP_PASS_TILE 4096
+#endif
+constexpr int kPassTile = SRPP_PASS_TILE;     // elements per tile of a digit pass (k_sort_pass)
 constexpr int kSortMinDigitBits = 5;          // >= 32 bins (one warp-row of the column scan)
 constexpr int kSortMaxDigitBits = 8;          // <= 256 bins: >= 16 elements per bin and tile, so the per-digit runs cover whole 32-byte sectors
 constexpr int kSortMaxBins = 1 << kSortMaxDigitBits;
