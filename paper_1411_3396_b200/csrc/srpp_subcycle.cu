@@ -205,14 +205,15 @@ __global__ void __launch_bounds__(256) k_merge_movers(
     const float4* __restrict__ pos, const float4* __restrict__ vel, const uint32_t* __restrict__ perm,
     const uint32_t* __restrict__ flag_words, const uint32_t* __restrict__ word_prefix, int64_t n,
     const uint32_t* __restrict__ cell_start, int64_t m, const uint32_t* __restrict__ m_key,
-    const uint32_t* __restrict__ m_idx, const uint32_t* __restrict__ m_slot, float4* __restrict__ pos_out,
+    const uint32_t* __restrict__ m_idx, const uint32_t* __restrict__ m_slot, const float4* __restrict__ m_pos_sorted,
+    float4* __restrict__ pos_out,
     float4* __restrict__ vel_out, uint32_t* __restrict__ perm_out) {
   const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= m) return;
   const uint32_t c = m_key[r], i = m_idx[r], src = m_slot[r];
   const uint32_t p = lower_bound_u32(perm, __ldg(&cell_start[c]), __ldg(&cell_start[c + 1]), i);
   const size_t dst = (size_t)p - movers_before(flag_words, word_prefix, p, (uint32_t)n, (uint32_t)m) + (size_t)r;
-  pos_out[dst] = pos[src];
+  pos_out[dst] = m_pos_sorted[r];          // the movers' sort already carried the positions: no gather through the old slot
   vel_out[dst] = vel[src];
   perm_out[dst] = i;
 }
@@ -341,7 +342,7 @@ extern "C" int32_t srpp_subcycle(srpp_ctx* c, float* pos_mass_f, float* vel_f, f
                                                   c->m_cell_start, c->mover_idx_sorted, c->sorted_buf[cur ^ 1], c->vel_s[cur ^ 1],
                                                   perm_new);
     k_merge_movers<<<(int)((m + 255) / 256), 256, 0, st>>>(c->sorted_buf[cur], c->vel_s[cur], c->perm, c->flag_words, c->prefix_f, n,
-                                                          c->cell_start, m, c->m_keys, c->mover_idx_sorted, c->mover_slot_sorted,
+                                                          c->cell_start, m, c->m_keys, c->mover_idx_sorted, c->mover_slot_sorted, c->m_sorted,
                                                           c->sorted_buf[cur ^ 1], c->vel_s[cur ^ 1], perm_new);
     k_new_cell_start<<<(c->geo.ncells + 1 + 255) / 256, 256, 0, st>>>(c->cell_start, c->geo.ncells, c->flag_words, c->prefix_f,
                                                                      (uint32_t)n, (uint32_t)m, c->m_cell_start);

@@ -80,6 +80,7 @@ def test_create_argument_errors(lib):
     # calls on a null context fail cleanly
     assert lib.srpp_build_mesh(None, None, 0) == -1
     assert lib.srpp_accel(None, None) == -1
+    assert lib.srpp_accel_kick(None, None, None, C.c_float(0.1)) == -1
     assert lib.srpp_get_mesh(None, None, None, None) == -1
     lib.srpp_destroy(None)
 

@@ -911,6 +911,13 @@ def test_new_entry_points_reject_bad_arguments(gpu):
     assert sol.lib.srpp_build_mesh(sol._ctx, buf.data_ptr() + 4, 100) == -1
     assert sol.lib.srpp_accel(sol._ctx, buf.data_ptr() + 8) == -1
     assert sol.lib.srpp_kick(sol._ctx, buf.data_ptr() + 4, buf.data_ptr(), C.c_float(0.1), 100) == -1
+    # srpp_accel_kick: misaligned / null pointers and a non-finite kdt are INVALID_ARG; before a mesh it is STATE
+    assert sol.lib.srpp_accel_kick(sol._ctx, buf.data_ptr() + 8, buf.data_ptr(), C.c_float(0.1)) == -1
+    assert sol.lib.srpp_accel_kick(sol._ctx, buf.data_ptr(), buf.data_ptr() + 4, C.c_float(0.1)) == -1
+    assert sol.lib.srpp_accel_kick(sol._ctx, buf.data_ptr(), None, C.c_float(0.1)) == -1
+    assert sol.lib.srpp_accel_kick(sol._ctx, buf.data_ptr(), buf.data_ptr(), C.c_float(float("nan"))) == -1
+    fresh = binding.Solver((32.0,) * 3, (10,) * 3, 3.0, 0.1, n_max=100)
+    assert fresh.lib.srpp_accel_kick(fresh._ctx, buf.data_ptr(), buf.data_ptr(), C.c_float(0.1)) == -5
     assert sol.lib.srpp_stream(sol._ctx, buf.data_ptr(), buf.data_ptr() + 4, C.c_float(0.1), 100) == -1
     torch.cuda.synchronize()
     pos = torch.rand((100, 4), device="cuda")
