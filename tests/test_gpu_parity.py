@@ -363,6 +363,35 @@ def test_accel_kick_fused_write_back(oracle_mod, gpu, n, ncell):
     print("accel_kick n=%d: per-particle max %.3e, global L2 %.3e" % (n, per, glob))
 
 
+@pytest.mark.parametrize("n", [(1 << 22) + 1, (1 << 22) + 4097])
+def test_write_back_bucketed_awkward_sizes(gpu, n):
+    """Property that holds at any size (the oracle check of the bucketed write-back is test_accel_kick_fused_write_back):
+    just above the 2^22 threshold, with a one-element and a one-element-past-a-tile tail, every destination is written
+    (NaN pre-fill), srpp_accel_kick equals srpp_accel + srpp_kick bit for bit, and re-ordering the input re-orders the
+    output (the intra-cell summation order follows the original index, hence a 1e-5 bound instead of equality)."""
+    torch, binding = gpu
+    ncell, box = (64, 64, 64), (3.2 * 64,) * 3
+    g = torch.Generator(device="cuda"); g.manual_seed(n)
+    pos = torch.rand((n, 4), generator=g, device="cuda") * (box[0] * 0.999999)
+    pos[:, 3] = 1.0
+    sol = binding.Solver(box, ncell, 3.0, 0.1, n_max=n)
+    sol.build_mesh(pos)
+    acc = torch.full((n, 4), float("nan"), device="cuda")
+    sol.accel(acc)
+    assert bool(torch.isfinite(acc).all())
+    vel = torch.randn((n, 4), generator=g, device="cuda")
+    v2, a2 = vel.clone(), torch.full((n, 4), float("nan"), device="cuda")
+    sol.accel_kick(v2, 0.02, acc=a2)
+    v1 = vel.clone()
+    sol.kick(v1, acc, 0.02)
+    assert torch.equal(a2, acc) and torch.equal(v1, v2)
+    shuf = torch.randperm(n, generator=g, device="cuda")
+    sol.build_mesh(pos[shuf].contiguous())
+    acc_s = sol.accel()
+    ref = acc[shuf]
+    assert float((acc_s - ref).abs().max() / ref.abs().max()) < 1e-5
+
+
 def test_subcycle_fixed_positions(oracle_mod, gpu):
     """Config-4 reading (R16): 5 x {build mesh, accel, kick} on fixed positions; identical accelerations each step
     are not required bit-wise (atomic order) but v5 = 5 kicks of the oracle's a within tolerance."""
