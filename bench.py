@@ -159,6 +159,9 @@ def _oracle_sample(oracle, pos, w, n_targets, seed):
     # candidates of target i in the WORKLOAD's mesh = stencil sum of its cell
     cid = oracle.cell_ids(pos[t], w.box, w.ncell)
     cand = sten.ravel()[cid].astype(np.int64)
+    # the harness logs how many cells hold half of W (the clustered W values are heavy-tail dominated)
+    ws = np.sort(w_cell)[::-1]
+    _oracle_sample.cells_half_w = int(np.searchsorted(np.cumsum(ws), 0.5 * ws.sum()) + 1)
     return t, cand
 
 
@@ -191,6 +194,7 @@ def oracle_rate(oracle, pos, w, budget_s: float, seed: int = 0):
     d_c = int(cand_all[:n_b].sum() - cand_all[:n_a].sum())
     rate = d_c / max(t_b - t_a, 1e-9)
     return {"value": rate, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "in_cutoff_fraction": frac_in,
+            "cells_holding_half_of_W": getattr(_oracle_sample, "cells_half_w", None),
             "sample": "%s: %d targets (half uniform, half work-weighted; SURVEY.md 8(d)), %d chaining-mesh candidate "
                       "pairs in %.1f s of fp64 oracle time; marginal rate between nested samples of %d and %d targets "
                       "(fixed cell-list build of %.1f s per call excluded)"
@@ -374,6 +378,7 @@ def run_product(args, w):
         line["phases"]["oracle_mesh_ms"] = 1e3 * (time.perf_counter() - t0)
         line["phases"]["oracle_mesh_kind"] = "orc_build_mesh, all %d particles, one host thread (plain counting sort)" % n
         frac = cb.pop("in_cutoff_fraction")
+        line["config"]["cells_holding_half_of_W"] = cb.pop("cells_holding_half_of_W")
         line["in_cutoff"] = {"fraction_of_candidates": frac, "pairs_per_s": value * frac,
                              "kind": "mean of n_in_i / candidates_i over the oracle's work-weighted target sample (= sum n_in / W in expectation)"}
         cb["full_config_extrapolated_s"] = W / cb["value"]
