@@ -461,6 +461,22 @@ def run_extras(args, torch, binding, dev, peak_tflops, peaks):
             torch.cuda.synchronize()
             rec["subcycle_ms_per_substep"] = ev0.elapsed_time(ev1) / 4
             del d_vel
+        if not args.no_cpu_baseline:
+            # oracle binning timed in full at every config; configs 1-2: the oracle evaluated in full
+            # (pairs/s = W / t and the exact in-cutoff pair count).  cpu_baseline leg: the one place this arm runs oracle/.
+            import oracle
+            oracle.build()
+            t0 = time.perf_counter()
+            oracle.build_mesh(pos, wc.box, wc.ncell)
+            rec["oracle_mesh_ms"] = 1e3 * (time.perf_counter() - t0)
+            if cfg <= 2:
+                t0 = time.perf_counter()
+                _, st_o = oracle.accel(pos, oracle.make_params(wc.box, wc.rcut, wc.eps), stats=True)
+                t_o = time.perf_counter() - t0
+                n_in = int(st_o["n_in"].sum())
+                rec["oracle_full"] = {"seconds": t_o, "pairs_per_s": W / t_o, "cores": oracle.num_threads(),
+                                      "in_cutoff_pairs": n_in, "in_cutoff_fraction_of_W": n_in / W,
+                                      "gpu_in_cutoff_pairs_per_s": n_in / (fm * 1e-3)}
         out["config%d" % cfg] = rec
         del sol, d_pos, d_acc
         torch.cuda.empty_cache()
