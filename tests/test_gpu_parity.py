@@ -392,6 +392,42 @@ def test_write_back_bucketed_awkward_sizes(gpu, n):
     assert float((acc_s - ref).abs().max() / ref.abs().max()) < 1e-5
 
 
+def test_write_back_three_levels_above_2p28(gpu):
+    """Maximum-size edge of the bucketed write-back: above 2^28 particles the destination index has more than 16
+    window bits and the partition takes three levels.  Properties that hold at any size (no oracle at this size):
+    every destination written, fused kick bit-identical, permutation invariance."""
+    torch, binding = gpu
+    n = (1 << 28) + 5003
+    free, _ = torch.cuda.mem_get_info()
+    if free < 80 * (1 << 30):
+        pytest.skip("needs ~60 GB of device memory")
+    ncell, box = (256, 256, 256), (3.2 * 256,) * 3
+    g = torch.Generator(device="cuda"); g.manual_seed(3)
+    pos = torch.rand((n, 4), generator=g, device="cuda") * (box[0] * 0.999999)
+    pos[:, 3] = 1.0
+    sol = binding.Solver(box, ncell, 3.0, 0.1, n_max=n)
+    sol.build_mesh(pos)
+    acc = torch.full((n, 4), float("nan"), device="cuda")
+    sol.accel(acc)
+    assert bool(torch.isfinite(acc).all())
+    vel = torch.zeros((n, 4), device="cuda")
+    v2, a2 = vel.clone(), torch.full((n, 4), float("nan"), device="cuda")
+    sol.accel_kick(v2, 0.5, acc=a2)
+    sol.kick(vel, acc, 0.5)
+    assert torch.equal(a2, acc) and torch.equal(vel, v2)
+    del a2, v2, vel
+    shuf = torch.randperm(n, generator=g, device="cuda")
+    pos_s = pos[shuf].contiguous()
+    del pos
+    sol.build_mesh(pos_s)
+    acc_s = sol.accel()
+    ref = acc[shuf]
+    del acc
+    assert float((acc_s - ref).abs().max() / ref.abs().max()) < 1e-5
+    del acc_s, ref, pos_s, shuf, sol
+    torch.cuda.empty_cache()
+
+
 def test_subcycle_fixed_positions(oracle_mod, gpu):
     """Config-4 reading (R16): 5 x {build mesh, accel, kick} on fixed positions; identical accelerations each step
     are not required bit-wise (atomic order) but v5 = 5 kicks of the oracle's a within tolerance."""
