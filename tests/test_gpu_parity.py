@@ -398,8 +398,9 @@ def test_write_back_three_levels_above_2p28(gpu):
     every destination written, fused kick bit-identical, permutation invariance."""
     torch, binding = gpu
     n = (1 << 28) + 5003
+    torch.cuda.empty_cache()                      # earlier tests' cached blocks do not count as free memory
     free, _ = torch.cuda.mem_get_info()
-    if free < 80 * (1 << 30):
+    if free < 64 * (1 << 30):
         pytest.skip("needs ~60 GB of device memory")
     ncell, box = (256, 256, 256), (3.2 * 256,) * 3
     g = torch.Generator(device="cuda"); g.manual_seed(3)
