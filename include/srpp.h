@@ -49,7 +49,8 @@ typedef enum {
   SRPP_ERR_WORKSPACE = -4,   /* workspace too small or not 256-byte aligned                                   */
   SRPP_ERR_STATE = -5,       /* srpp_accel before a successful srpp_build_mesh, n mismatch, or the current CUDA
                                 device is not the one the context was created on                             */
-  SRPP_ERR_CUDA = -6         /* CUDA runtime error (text of the last one: srpp_last_cuda_error)                */
+  SRPP_ERR_CUDA = -6,        /* CUDA runtime error (text of the last one: srpp_last_cuda_error)                */
+  SRPP_ERR_LIMIT = -7        /* a size beyond the fixed capacity of srpp_mbp_static's built-in scratch array     */
 } srpp_status;
 
 /* Solver parameters (plain data; copied by srpp_create). */
@@ -176,6 +177,29 @@ int32_t srpp_set_boundary(srpp_ctx* ctx, const int32_t* periodic_host, const flo
 int32_t srpp_mbp_workspace_bytes(int64_t n, int64_t nhalo, size_t* bytes_host);
 int32_t srpp_mbp(srpp_ctx* ctx, const float* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo,
                  float* phi, int64_t* mbp_index, float* mbp_phi, void* workspace, size_t workspace_bytes);
+
+/* srpp_mbp for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same computation as srpp_mbp -- same kernels, same reading R19, same outputs --
+ * but with NO workspace argument and no context.  The scratch memory (fp64 potential accumulators, the halo table, the work-item
+ * prefix, the queue counter) lives in one static __device__ array inside the library, sized for
+ *     n <= SRPP_MBP_STATIC_MAX_N (2^20 members)  and  nhalo <= SRPP_MBP_STATIC_MAX_HALOS (2^16 halos),
+ * about 9.1 MB, which every GPU that loads the library holds until the process exits.  A larger n or nhalo is rejected with
+ * SRPP_ERR_LIMIT (use srpp_mbp with a caller-owned workspace instead).  The call allocates nothing: no cudaMalloc, no cudaFree,
+ * no allocating library routine; it only enqueues memsets, one copy of the halo table and the kernels on `cuda_stream`.
+ *   pos_mass, phi, mbp_index, mbp_phi, halo_start_host   as for srpp_mbp (phi and mbp_phi may be NULL)
+ *   eps               Plummer softening length (> 0, finite); srpp_mbp takes it from its context
+ *   cuda_stream       cudaStream_t as void* (0 = the legacy default stream); asynchronous, no synchronisation
+ * The array is SHARED by every call on a device and keeps the last call's contents; each call clears the parts that must
+ * start at zero (queue counter, accumulators of the n members it uses).  Two calls whose GPU work overlaps (different
+ * streams, or host threads that do not order their calls) RACE on it: order them on one stream or with events.
+ * The first call on each device looks the array's device address up (cudaGetSymbolAddress, with that device current) and
+ * queries the SM count and the kernel's occupancy; make that first call outside a stream capture.
+ * Errors: INVALID_ARG (null / misaligned pointer, n or nhalo < 0, eps <= 0 or non-finite, halo table not monotone or beyond n),
+ * LIMIT (n or nhalo above the maxima), STATE (device index above 63), CUDA. */
+#define SRPP_MBP_STATIC_MAX_N (1 << 20)
+#define SRPP_MBP_STATIC_MAX_HALOS (1 << 16)
+int32_t srpp_mbp_static(const float* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo, float eps,
+                        float* phi, int64_t* mbp_index, float* mbp_phi, void* cuda_stream);
 
 /* Block decomposition of the node volume with the x2 adaptive refinement rule (PAPER.md:73-77:
  * "1) Each node partitions itself into overlapping data blocks, 2) evolves the blocks independently, and 3) reconciles the

@@ -15,12 +15,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsrpp.so")
 
 SRPP_OK = 0
-STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "GEOMETRY", -3: "DOMAIN", -4: "WORKSPACE", -5: "STATE", -6: "CUDA"}
+STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "GEOMETRY", -3: "DOMAIN", -4: "WORKSPACE", -5: "STATE", -6: "CUDA", -7: "LIMIT"}
+MBP_STATIC_MAX_N, MBP_STATIC_MAX_HALOS = 1 << 20, 1 << 16      # include/srpp.h
 
 EXPORTS = ("srpp_version", "srpp_default_poly", "srpp_workspace_bytes", "srpp_create", "srpp_destroy",
            "srpp_build_mesh", "srpp_get_mesh", "srpp_accel", "srpp_accel_kick", "srpp_get_stats", "srpp_kick", "srpp_stream",
            "srpp_step_host", "srpp_strerror", "srpp_last_cuda_error", "srpp_set_timing", "srpp_get_timings",
-           "srpp_probe_fp32", "srpp_set_boundary", "srpp_mbp_workspace_bytes", "srpp_mbp", "srpp_subcycle",
+           "srpp_probe_fp32", "srpp_set_boundary", "srpp_mbp_workspace_bytes", "srpp_mbp", "srpp_mbp_static", "srpp_subcycle",
            "srpp_blocks_workspace_bytes", "srpp_blocks_init", "srpp_accel_blocks", "srpp_get_blocks")
 
 
@@ -111,6 +112,8 @@ def load() -> C.CDLL:
     L.srpp_mbp_workspace_bytes.argtypes = [i64, i64, C.POINTER(C.c_size_t)]
     L.srpp_mbp.restype = i32
     L.srpp_mbp.argtypes = [vp, vp, i64, C.POINTER(i64), i64, vp, vp, vp, vp, C.c_size_t]
+    L.srpp_mbp_static.restype = i32
+    L.srpp_mbp_static.argtypes = [vp, i64, C.POINTER(i64), i64, f32, vp, vp, vp, vp]
     L.srpp_set_boundary.restype = i32
     L.srpp_set_boundary.argtypes = [vp, C.POINTER(i32), C.POINTER(C.c_float), C.POINTER(C.c_float)]
     L.srpp_probe_fp32.restype = i32
@@ -153,6 +156,24 @@ def workspace_bytes(params: SrppParams, n: int) -> int:
 
 def strerror(status: int) -> str:
     return load().srpp_strerror(int(status)).decode()
+
+
+def mbp_static(pos_mass, halo_start, eps: float, idx, pmin=None, phi=None, stream=None) -> None:
+    """srpp_mbp_static: the most bound particle of every halo with the library's built-in scratch array -- no workspace,
+    no context, no device allocation.  The caller passes every output: idx int64 [nhalo], pmin float32 [nhalo] or None,
+    phi float32 [n] or None (CUDA tensors).  halo_start: host int64 sequence [nhalo+1].  Raises SrppError (status -7 =
+    LIMIT above MBP_STATIC_MAX_N members or MBP_STATIC_MAX_HALOS halos)."""
+    hs = np.ascontiguousarray(halo_start, dtype=np.int64)
+    nh, n = int(hs.shape[0]) - 1, int(pos_mass.shape[0])
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream(pos_mass.device)
+    st = stream.cuda_stream
+    rc = load().srpp_mbp_static(pos_mass.data_ptr(), n, hs.ctypes.data_as(C.POINTER(C.c_int64)), nh, float(eps),
+                                phi.data_ptr() if phi is not None else None, idx.data_ptr() if nh > 0 else None,
+                                pmin.data_ptr() if pmin is not None else None, st)
+    if rc != SRPP_OK:
+        raise SrppError(rc, "srpp_mbp_static", strerror(rc))
 
 
 class Solver:

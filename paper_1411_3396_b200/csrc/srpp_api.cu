@@ -461,6 +461,7 @@ const char* srpp_strerror(int32_t s) {
     case SRPP_ERR_WORKSPACE: return "workspace too small or misaligned";
     case SRPP_ERR_STATE: return "state: no valid chaining mesh (call srpp_build_mesh first)";
     case SRPP_ERR_CUDA: return "CUDA runtime error";
+    case SRPP_ERR_LIMIT: return "limit: size beyond the capacity of the built-in scratch array (srpp_mbp_static)";
     default: return "unknown status";
   }
 }

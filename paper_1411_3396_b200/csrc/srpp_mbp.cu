@@ -13,7 +13,11 @@
 //   * the self pair is included in the stream (d = 0 exactly, term m_i * rsqrt(eps^2)) and removed afterwards;
 //   * <= 1024 fp32 terms per item, folded into fp64 with red.global.add.f64; a second kernel negates, removes the self
 //     term and reduces (phi, index) per halo.
+#include <math.h>
+#include <string.h>
+
 #include <algorithm>
+#include <mutex>
 
 #include "srpp_internal.cuh"
 
@@ -207,3 +211,81 @@ cudaError_t launch_mbp(srpp_ctx* c, const float4* pos_mass, int64_t n, const int
 }
 
 }  // namespace srpp
+
+// --------------------------------------------------------------- srpp_mbp_static: no allocation --
+// The same launch sequence as srpp_mbp (launch_mbp above, unchanged), for callers that cannot allocate device memory:
+// the workspace is a static __device__ array of this translation unit instead of a caller allocation.  Capacity:
+// SRPP_MBP_STATIC_MAX_N members and SRPP_MBP_STATIC_MAX_HALOS halos (include/srpp.h), laid out by mbp_workspace_layout.
+constexpr size_t mbp_up256(size_t x) { return (x + 255) / 256 * 256; }
+constexpr size_t kMbpStaticBytes = 256 + mbp_up256(8 * (size_t)SRPP_MBP_STATIC_MAX_N) +
+                                   2 * mbp_up256(8 * ((size_t)SRPP_MBP_STATIC_MAX_HALOS + 1)) +
+                                   mbp_up256(8 * ((size_t)SRPP_MBP_STATIC_MAX_HALOS / 4096 + 2));
+
+// ~9.1 MB on every GPU that loads the library, until the process exits.  In HOST code this name is only a stand-in for
+// the symbol, not a device address: the address is looked up once per device with cudaGetSymbolAddress (below).
+static __device__ __align__(256) unsigned char g_mbp_static_scratch[kMbpStaticBytes];
+
+namespace {
+
+constexpr int kMbpStaticMaxDevices = 64;
+struct MbpStaticDevice {
+  char* ws;        // device address of g_mbp_static_scratch on this device
+  int num_sms;
+  int occ;         // resident CTAs per SM of k_mbp_phi (0 = not queried yet)
+  bool ready;
+};
+MbpStaticDevice g_mbp_static_dev[kMbpStaticMaxDevices];
+std::mutex g_mbp_static_mutex;
+
+}  // namespace
+
+extern "C" int32_t srpp_mbp_static(const float* pos_mass, int64_t n, const int64_t* halo_start_host, int64_t nhalo, float eps,
+                                   float* phi, int64_t* mbp_index, float* mbp_phi, void* cuda_stream) {
+  if (n < 0 || nhalo < 0 || !halo_start_host || (n > 0 && !pos_mass) || (nhalo > 0 && !mbp_index) ||
+      ((uintptr_t)pos_mass & 15u) != 0 || !(eps > 0.f) || !isfinite(eps))
+    return SRPP_ERR_INVALID_ARG;
+  if (n > (int64_t)SRPP_MBP_STATIC_MAX_N || nhalo > (int64_t)SRPP_MBP_STATIC_MAX_HALOS) return SRPP_ERR_LIMIT;
+  if (halo_start_host[0] < 0 || halo_start_host[nhalo] > n) return SRPP_ERR_INVALID_ARG;
+  for (int64_t h = 0; h < nhalo; ++h)
+    if (halo_start_host[h + 1] < halo_start_host[h]) return SRPP_ERR_INVALID_ARG;
+  size_t a, b, d, t;
+  if (srpp::mbp_workspace_layout(n, nhalo, &a, &b, &d, &t) > kMbpStaticBytes) return SRPP_ERR_LIMIT;   // (cannot happen below the maxima)
+
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SRPP_ERR_CUDA;
+  if (dev < 0 || dev >= kMbpStaticMaxDevices) return SRPP_ERR_STATE;
+  MbpStaticDevice info;
+  {
+    // set-up, once per device, with that device current: the array's device address, the SM count
+    std::lock_guard<std::mutex> lock(g_mbp_static_mutex);
+    MbpStaticDevice& s = g_mbp_static_dev[dev];
+    if (!s.ready) {
+      char* ptr = nullptr;
+      if (cudaGetSymbolAddress((void**)&ptr, g_mbp_static_scratch) != cudaSuccess || !ptr) return SRPP_ERR_CUDA;
+      int sms = 0;
+      if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) return SRPP_ERR_CUDA;
+      s.ws = ptr;
+      s.num_sms = sms;
+      s.occ = 0;
+      s.ready = true;
+    }
+    info = s;
+  }
+
+  // launch_mbp reads only these fields of a context: stream, eps^2, SM count, cached occupancy, launch counter
+  srpp_ctx tmp;
+  memset(&tmp, 0, sizeof(tmp));
+  tmp.stream = (cudaStream_t)cuda_stream;
+  tmp.device = dev;
+  tmp.num_sms = info.num_sms;
+  tmp.mbp_occ = info.occ;
+  tmp.fc.eps2 = (float)((double)eps * (double)eps);      // as srpp_create computes it
+  const cudaError_t e = srpp::launch_mbp(&tmp, (const float4*)pos_mass, n, halo_start_host, nhalo, phi, (long long*)mbp_index,
+                                         mbp_phi, info.ws);
+  if (e != cudaSuccess) return SRPP_ERR_CUDA;
+  if (!info.occ && tmp.mbp_occ) {
+    std::lock_guard<std::mutex> lock(g_mbp_static_mutex);
+    g_mbp_static_dev[dev].occ = tmp.mbp_occ;
+  }
+  return SRPP_OK;
+}
